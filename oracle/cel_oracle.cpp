@@ -696,9 +696,15 @@ void phase_push(Oracle& o) {
 }
 
 // ---------------------------------------------------------------- one step iteration (S1)
+void phases_after_reindex(Oracle& o);
+
 void step_iteration(Oracle& o) {
   phase_init(o);
   phase_reindex(o);
+  phases_after_reindex(o);
+}
+
+void phases_after_reindex(Oracle& o) {
   // record the tally bin of the volume at the start of the iteration
   for (uint64_t s = 0; s < o.n_slots; ++s) {
     const OrcTrack& t = o.tracks[s];
@@ -784,6 +790,10 @@ int orc_begin(void* h, const OrcPrimary* prim, uint64_t n, uint32_t n_events) {
 }
 
 int orc_step(void* h) { Oracle& o = *(Oracle*)h; step_iteration(o); return o.error; }
+// the same iteration in three pieces, so that a test can look at the state between phases
+void orc_phase_init(void* h) { phase_init(*(Oracle*)h); }
+void orc_phase_reindex(void* h) { phase_reindex(*(Oracle*)h); }
+int orc_phase_rest(void* h) { Oracle& o = *(Oracle*)h; phases_after_reindex(o); return o.error; }
 
 // run to completion (alive == 0 and I == 0) or max_iter iterations; returns iterations executed or <0
 int64_t orc_run(void* h, uint64_t max_iter) {

@@ -54,6 +54,9 @@ def lib():
         L.orc_n_bins.argtypes = [C.c_void_p]
         L.orc_begin.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32]
         L.orc_step.argtypes = [C.c_void_p]
+        L.orc_phase_init.argtypes = [C.c_void_p]
+        L.orc_phase_reindex.argtypes = [C.c_void_p]
+        L.orc_phase_rest.argtypes = [C.c_void_p]
         L.orc_run.restype = C.c_int64
         L.orc_run.argtypes = [C.c_void_p, C.c_uint64]
         for name in ("orc_read_state", "orc_read_counts", "orc_read_initializers", "orc_read_tallies", "orc_read_counters"):
@@ -179,6 +182,17 @@ class Oracle:
         rc = lib().orc_step(self.h)
         if rc != 0:
             raise RuntimeError(f"orc_step failed: {rc}")
+
+    def phase_init(self):
+        lib().orc_phase_init(self.h)
+
+    def phase_reindex(self):
+        lib().orc_phase_reindex(self.h)
+
+    def phase_rest(self):
+        rc = lib().orc_phase_rest(self.h)
+        if rc != 0:
+            raise RuntimeError(f"orc_phase_rest failed: {rc}")
 
     def run(self, max_iter=1 << 40):
         n = lib().orc_run(self.h, max_iter)

@@ -1,0 +1,168 @@
+"""Pins of the CPU oracle against things other than itself: PRNG known answers, cross-section
+closed forms and quadratures, table values (spec S3, S4). No GPU."""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate, stats
+
+import oracle as orc
+from helpers import golden_values, make_oracle, rel_close, HERE
+from paper_2503_17608_b200 import workloads as W
+
+G = golden_values()
+M_E = 0.51099895
+R_E = 2.8179403262e-13
+MATS = [W.LEAD, W.LAR, W.SILICON, W.PBWO4, W.BRASS]
+NAMES = ["Pb", "LAr", "Si", "PbWO4", "brass"]
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    geo = W.slab_geometry([0.0, 1.0], [0], [0], 50.0)
+    return orc.Oracle(geo, MATS, W.physics(1), 64, 1)
+
+
+def test_philox_known_answers():
+    with open(os.path.join(HERE, "golden", "philox4x32_10_kat.txt")) as f:
+        rows = [l.split() for l in f if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = orc.philox(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_uniform_mapping_worked_example():
+    # SURVEY.md S3 worked mapping: counter=(5,0,1,0), key=(1,0) -> xi = 0.611825928356205
+    w = orc.philox([5, 0, 1, 0], [1, 0])
+    assert [int(x) for x in w] == [578703075, 2627772353, 2538312612, 1332725330]
+    x = (int(w[1]) << 32) | int(w[0])
+    xi = ((x >> 12) + 0.5) / 2.0 ** 52
+    assert orc.uniform(1, 5, 0, 1, 0) == xi
+    assert abs(xi - 0.611825928356205) < 1e-15
+    x1 = (int(w[3]) << 32) | int(w[2])
+    assert orc.uniform(1, 5, 0, 1, 1) == ((x1 >> 12) + 0.5) / 2.0 ** 52
+    # draw 2 comes from block 1
+    w2 = orc.philox([5, 0, 1, 1], [1, 0])
+    assert orc.uniform(1, 5, 0, 1, 2) == ((((int(w2[1]) << 32) | int(w2[0])) >> 12) + 0.5) / 2.0 ** 52
+    # 64-bit seed goes to both key words
+    w3 = orc.philox([7, 3, 2, 0], [0xdeadbeef, 0x12345678])
+    assert orc.uniform(0x12345678deadbeef, 7, 3, 2, 0) == ((((int(w3[1]) << 32) | int(w3[0])) >> 12) + 0.5) / 2.0 ** 52
+
+
+def test_uniform_statistics():
+    n = 200000
+    u = np.array([orc.uniform(9, i, 3, 1, 0) for i in range(n)])
+    assert u.min() > 0.0 and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 4 * (1 / math.sqrt(12 * n))
+    h, _ = np.histogram(u, bins=100, range=(0, 1))
+    assert stats.chisquare(h).pvalue > 1e-4
+    # streams of neighbouring slots / iterations are uncorrelated
+    v = np.array([orc.uniform(9, i + 1, 3, 1, 0) for i in range(n)])
+    assert abs(np.corrcoef(u, v)[0, 1]) < 4 / math.sqrt(n)
+
+
+def kn_dsigma_domega(E, cost):
+    k = E / M_E
+    r = 1.0 / (1.0 + k * (1.0 - cost))
+    return 0.5 * R_E ** 2 * r * r * (r + 1.0 / r - (1.0 - cost * cost))
+
+
+@pytest.mark.parametrize("E", [1e-3, 1e-2, 0.1, 0.511, 1.0, 10.0, 1e3, 1e5])
+def test_sigma_kn_vs_quadrature_of_differential(E):
+    val, err = integrate.quad(lambda c: 2 * math.pi * kn_dsigma_domega(E, c), -1, 1, epsabs=0, epsrel=1e-12, limit=200)
+    tol = 1e-9 + 4e-16 / (E / M_E) ** 2 * 10  # cancellation of the closed form at small k (spec S4 note)
+    assert rel_close(orc.sigma_kn(E), val, tol)
+
+
+def test_sigma_kn_golden_and_thomson():
+    sT = 8 * math.pi * R_E ** 2 / 3
+    assert rel_close(sT, *G["sigma_T_cm2"])
+    assert rel_close(orc.sigma_kn(1e-3) / sT, *G["sigma_KN_1keV_over_sigma_T"])
+    assert rel_close(orc.sigma_kn(1.0), *G["sigma_KN_1MeV_cm2"])
+    # Thomson limit: sigma -> sigma_T (1 - 2k) as k -> 0
+    k = 1e-4
+    assert abs(orc.sigma_kn(k * M_E) / sT - (1 - 2 * k)) < 1e-6
+
+
+def test_lead_1MeV_cross_sections(ctx):
+    assert abs(ctx.lookup(0, "pe", 1.0) - 1.0) < 1e-13          # normalisation (BASELINE.json config 1)
+    assert rel_close(ctx.lookup(0, "compton", 1.0), *G["Sigma_C_Pb_1MeV"])
+    mu = ctx.lookup(0, "pe", 1.0) + ctx.lookup(0, "compton", 1.0)
+    assert rel_close(mu, *G["mu_Pb_1MeV"])
+    # PE scaling laws: E^-3.5 and Z^5 per atom
+    assert rel_close(ctx.table(0, "pe")[192 + 64] / ctx.table(0, "pe")[192], 10 ** -3.5, 1e-12)
+    n_pb = 11.35 / 207.2
+    n_si = 2.33 / 28.09
+    assert rel_close(ctx.table(2, "pe")[192], (n_si / n_pb) * (14 / 82) ** 5, 1e-12)
+
+
+def test_grid_nodes(ctx):
+    # 1 MeV is node 192; the grid spans 1 keV .. 1e6 MeV with 64 nodes per decade
+    t = ctx.table(0, "brems")
+    x0 = 1.0 / ctx.inv_X0(0)
+    assert abs(t[0]) < 1e-12
+    assert rel_close(t[192], math.log(1e3) / x0, 1e-12)
+    assert rel_close(t[576], math.log(1e9) / x0, 1e-12)
+    # brems table is linear in u, so the lerp is exact
+    assert rel_close(ctx.lookup(0, "brems", 3.3), math.log(3.3e3) / x0, 1e-12)
+
+
+def test_radiation_lengths(ctx):
+    for i, n in enumerate(NAMES):
+        assert rel_close(1.0 / ctx.inv_X0(i), *G[f"X0_{n}_cm"])
+    assert rel_close(1.0 / ctx.lookup(0, "brems", 1e4), *G["brems_mfp_Pb_10GeV_cm"])
+    assert rel_close(1.0 / ctx.lookup(0, "brems", 10.0), *G["brems_mfp_Pb_10MeV_cm"])
+
+
+def test_pair_cross_section(ctx):
+    assert ctx.lookup(0, "pair", 3.0) == 0.0
+    assert ctx.lookup(0, "pair", 1.0) == 0.0
+    for key, E in (("5MeV", 5.0), ("10MeV", 10.0), ("100MeV", 100.0), ("1GeV", 1e3)):
+        assert rel_close(ctx.lookup(0, "pair", E), *G[f"Sigma_pair_Pb_{key}"])
+    assert rel_close(ctx.lookup(1, "pair", 1e3), *G["Sigma_pair_LAr_1GeV"])
+    # threshold of the no-screening form: (28/9) ln(2E/m) = 218/27
+    thr = 0.5 * M_E * math.exp(218 / 27 * 9 / 28)
+    assert abs(thr - 3.4236) < 1e-4
+    tab = ctx.table(0, "pair")
+    E = np.exp(math.log(1e-3) + np.arange(577) * math.log(10) / 64)
+    assert np.all(tab[E <= thr] == 0.0) and np.all(tab[E > thr * 1.04] > 0.0)
+    assert np.all(np.diff(tab) >= 0)
+
+
+def test_stopping_power_golden(ctx):
+    for i, n in enumerate(NAMES):
+        assert rel_close(ctx.stopping_power(i, 1.0), *G[f"S_{n}_1MeV"])
+    assert rel_close(ctx.stopping_power(0, 1e4), *G["S_Pb_10GeV"])
+    # positive on the whole grid for every material
+    for i in range(5):
+        for E in np.logspace(-3, 6, 200):
+            assert ctx.stopping_power(i, E) > 0
+
+
+def test_csda_range_vs_adaptive_quadrature(ctx):
+    """BASELINE.json north_star pin 3: CSDA range against numerical integration of 1/S."""
+    cases = [(0, "Pb", [0.01, 0.1, 1, 10, 100]), (1, "LAr", [1, 10, 100]), (2, "Si", [1]), (3, "PbWO4", [1]), (4, "brass", [1])]
+    for mat, name, energies in cases:
+        for T in energies:
+            # independent integrator (QUADPACK adaptive Gauss-Kronrod in T, not Simpson in u)
+            pts = [p for p in (1e-2, 1e-1, 1, 10) if 1e-3 < p < T]
+            val, _ = integrate.quad(lambda x: 1.0 / ctx.stopping_power(mat, x), 1e-3, T, epsabs=0, epsrel=1e-12, limit=500, points=pts or None)
+            r_tab = ctx.lookup(mat, "range", T)          # these energies are grid nodes
+            assert rel_close(r_tab, val, 1e-9), (name, T, r_tab, val)
+            key = f"R_{name}_{T:g}MeV"
+            if key in G:
+                assert rel_close(r_tab, *G[key]), key
+
+
+def test_range_inverse_is_exact_inverse(ctx):
+    rng = np.random.default_rng(0)
+    for mat in range(5):
+        for T in np.exp(rng.uniform(math.log(1.1e-3), math.log(9e5), 200)):
+            r = ctx.lookup(mat, "range", T)
+            assert rel_close(ctx.range_inverse(mat, r), T, 2e-12)
+    # monotone
+    for mat in range(5):
+        assert np.all(np.diff(ctx.table(mat, "range")) > 0)
