@@ -1,0 +1,141 @@
+/* cel.h — C ABI of celstep, the B200-native step iteration over a struct-of-arrays array of track slots.
+ *
+ * What the calls are: the paper's statement of the problem (arXiv 2503.17608): a *step iteration* over a
+ * large array of track slots (section 2), with the optional reindexing of slot indices
+ * `state[state_indices[tid]]` (section 3.1), a cap on field substeps (section 3.3)
+ * and stream-ordered memory so that the host never blocks (section 3.4), in the "standalone
+ * application" model where all events are mixed in one track array. BASELINE.json's north_star
+ * names the three calls cel_create / cel_transport / cel_tallies; the physics is docs/PHYSICS_SPEC.md.
+ *
+ * Conventions. Units: MeV, cm, tesla. All structs are plain C in HOST memory and are copied during the call
+ * (the caller keeps ownership). Every call returns 0 (CEL_OK) or a negative CEL_ERR_* code; nothing throws
+ * across the ABI; there is no global state; a context must be used from one host thread at a time.
+ * All device work is enqueued on the context's stream (its own, or the one given by cel_set_stream).
+ * There is no CPU fallback: without a CUDA device cel_create fails with CEL_ERR_CUDA.
+ */
+#ifndef CEL_H
+#define CEL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cel_ctx cel_ctx; /* opaque; owned by the library; freed by cel_destroy */
+
+enum { CEL_SORT_NONE = 0, CEL_SORT_BY_ACTION = 1, CEL_SORT_BY_PARTICLE = 2 };
+enum { CEL_GEOM_SLAB = 0, CEL_GEOM_CYL = 1 };
+enum { CEL_GAMMA = 0, CEL_ELECTRON = 1, CEL_POSITRON = 2 };
+/* action IDs = sort keys (docs/PHYSICS_SPEC.md S2) */
+enum { CEL_ACT_PE = 0, CEL_ACT_PAIR = 1, CEL_ACT_COMPTON = 2, CEL_ACT_MOVE_G = 3, CEL_ACT_MOVE_C = 4,
+       CEL_ACT_BREMS = 5, CEL_ACT_ANNIH = 6, CEL_ACT_VACANT = 7 };
+
+enum {
+  CEL_OK = 0,
+  CEL_ERR_INVALID_ARG = -1,   /* null pointer, bad enum, non-unit direction, primary outside the geometry, ... */
+  CEL_ERR_CUDA = -2,          /* a CUDA runtime call failed (cel_last_cuda_error gives the text) */
+  CEL_ERR_OOM = -3,           /* device or pinned allocation failed */
+  CEL_ERR_INIT_OVERFLOW = -4, /* initializer stack exceeded init_capacity (S9); results invalid */
+  CEL_ERR_TALLY_OVERFLOW = -5,
+  CEL_ERR_NONFINITE = -6,     /* a non-finite energy or position was produced */
+  CEL_ERR_NOT_RUN = -7,       /* cel_tallies before any cel_transport */
+  CEL_ERR_MAX_ITER = -8       /* the run did not end within max_iterations */
+};
+
+/* one effective element per material (S0) */
+typedef struct { double density_g_cm3, Z, A; } cel_material;
+
+typedef struct {
+  int kind;                /* CEL_GEOM_SLAB: bounds = z planes. CEL_GEOM_CYL: bounds = radii, bounds[0] = 0 (S6) */
+  int n_vol;               /* 1..254 */
+  const double* bounds;    /* host, n_vol+1 ascending values */
+  const int* vol_material; /* host, n_vol entries, index into mats or -1 = vacuum */
+  const int* vol_bin;      /* host, n_vol entries, tally bin or -1 = not scored */
+  double half_x, half_y;   /* slab half-widths */
+  double half_z;           /* cylinder half-length */
+  double field_T[3];       /* uniform field; all zero = no field */
+} cel_geometry;
+
+typedef struct {
+  uint64_t seed;           /* Philox key (S3) */
+  double cut_MeV;          /* production and tracking cut; the table grid starts at 1e-3 MeV (S4) */
+  int enable_pair, enable_brems, enable_msc, enable_eloss, enable_annihilation;
+  int electrons_local;     /* 1 = every electron is deposited where it is born (config 1) */
+  int max_substeps;        /* field substeps per iteration, 10 in the paper */
+  uint32_t max_steps_per_track; /* looper kill (S7.6) */
+  uint64_t init_capacity;  /* initializer stack capacity; 0 = max(8 n_slots, 2^24) */
+} cel_physics;
+
+/* 64 bytes */
+typedef struct { uint32_t event; int32_t ptype; double energy_MeV; double pos[3]; double dir[3]; } cel_primary;
+
+/* unpacked view of one track slot or one initializer (debug surface), 80 bytes */
+typedef struct {
+  double pos[3]; double dir[3]; double energy;
+  uint32_t event; uint32_t nsteps; int32_t vol; int32_t surf; int32_t ptype; int32_t action;
+} cel_track;
+
+typedef struct {
+  uint32_t n_events; int32_t n_bins;  /* bin n_bins = escaped energy */
+  const uint64_t* fixed;              /* [n_events][n_bins+1], units 2^-36 MeV; library-owned pinned HOST memory,
+                                         valid until the next cel_transport / cel_destroy */
+  uint64_t track_steps, iterations, secondaries; /* S11 */
+  double seconds;                     /* device time of the last cel_transport (CUDA events on the stream) */
+  uint64_t kernel_launches;           /* kernels enqueued by the last cel_transport */
+} cel_tally_view;
+
+/* Create a context: builds the physics tables on the host (S4), uploads geometry and tables, allocates the
+ * SoA state for n_slots slots (N <= 2^31), the staging areas and the initializer stack. mats: n_mats entries.
+ * sort_mode: CEL_SORT_*. On success *out owns device memory until cel_destroy. */
+int cel_create(const cel_geometry* geometry, const cel_material* mats, int n_mats, const cel_physics* physics,
+               uint64_t n_slots, int sort_mode, cel_ctx** out);
+
+/* Use the caller's CUDA stream (a cudaStream_t passed as void*, e.g. torch.cuda.current_stream().cuda_stream).
+ * Must be called before the first cel_transport / cel_debug_begin; the stream must outlive the context. */
+int cel_set_stream(cel_ctx*, void* cuda_stream);
+
+/* Bytes of device workspace cel_create would allocate for these sizes; cel_set_workspace lets the caller own
+ * that memory instead (e.g. a torch tensor): dptr is a DEVICE pointer, 256-byte aligned, bytes >= the size
+ * reported; it must outlive the context and must be set before the first transport. */
+uint64_t cel_workspace_bytes(uint64_t n_slots, uint64_t init_capacity, int sort_mode);
+int cel_set_workspace(cel_ctx*, void* dptr, uint64_t bytes);
+
+/* Transport: resets slots, tallies (sized n_events x (n_bins+1)) and counters, writes primary i to init[i]
+ * (S9; primaries is a HOST array, validated, copied), then enqueues step iterations in batches on the stream
+ * and returns when a lagged, asynchronously copied status word shows that no track and no initializer is left.
+ * The host never issues a synchronous copy or a device-wide synchronisation. */
+int cel_transport(cel_ctx*, const cel_primary* primaries, uint64_t n_primaries, uint32_t n_events);
+
+/* Same, but the primaries are already resident in DEVICE memory as n_primaries packed cel_primary records
+ * (validated by the caller); used to time the path with inputs in HBM. */
+int cel_transport_device(cel_ctx*, const void* d_primaries, uint64_t n_primaries, uint32_t n_events);
+
+/* Synchronises the stream, copies the integer tallies to pinned host memory and fills *out. */
+int cel_tallies(cel_ctx*, cel_tally_view* out);
+
+void cel_destroy(cel_ctx*);
+const char* cel_strerror(int code);
+const char* cel_last_cuda_error(cel_ctx*);
+
+/* Run-time knobs (before a transport). use_graph: replay one captured CUDA graph per iteration (default 1).
+ * batch: iterations enqueued between status polls (default 16). max_iterations: safety stop (default 2^22). */
+int cel_set_option(cel_ctx*, const char* name, int64_t value);
+
+/* ---- debug / parity surface (synchronous, not timed) ---- */
+int cel_debug_begin(cel_ctx*, const cel_primary* primaries, uint64_t n, uint32_t n_events); /* load only */
+int cel_debug_step(cel_ctx*);                                 /* exactly one step iteration, then synchronise */
+int cel_debug_read_state(cel_ctx*, cel_track* host_out);      /* n_slots records */
+int cel_debug_read_indices(cel_ctx*, uint32_t* idx /* n_slots */, uint32_t* offsets /* 9 */);
+int cel_debug_n_initializers(cel_ctx*, uint64_t* n);
+int cel_debug_read_initializers(cel_ctx*, cel_track* host_out /* n records, action = -1 */);
+int cel_debug_n_counts(cel_ctx*, uint64_t* n_iterations_logged);
+int cel_debug_read_counts(cel_ctx*, uint32_t* host_out /* [n][8] */);
+int cel_debug_table(cel_ctx*, int material, int which /* 0 C, 1 PE, 2 pair, 3 brems, 4 range */, double* out577);
+int cel_debug_uniforms(cel_ctx*, const uint32_t* slots, uint32_t n, uint32_t k, uint32_t phase, uint32_t j,
+                       double* host_out);                     /* xi_j(seed, slot, k, phase) evaluated on the device */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CEL_H */

@@ -1,0 +1,681 @@
+// cel_api.cu — host side of the celstep C ABI (include/cel.h): context, physics tables (docs/PHYSICS_SPEC.md S4),
+// HBM layout, the non-blocking step-iteration loop and the debug/parity surface.
+// No torch types, no CPU fallback: every step of the path runs in the kernels of cel_kernels.cuh.
+#include "../../include/cel.h"
+#include "cel_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace cel;
+
+static_assert(sizeof(cel_primary) == 64 && sizeof(PrimaryRec) == 64, "cel_primary layout");
+static_assert(sizeof(cel_track) == 80 && sizeof(TrackRec) == 80, "cel_track layout");
+static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32 && sizeof(Stage) == 32, "record layout");
+static_assert(sizeof(DeviceState) < 3500, "DeviceState must fit in kernel parameter space");
+
+namespace {
+
+constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action counts are logged
+constexpr int kStatusSlots = 2;
+
+struct HostTables {                 // per material, kept for cel_debug_table
+  std::vector<double> t[5];         // compton, pe, pair, brems, range
+  double inv_X0;
+};
+
+}  // namespace
+
+struct cel_ctx {
+  DeviceState D{};
+  int n_mats = 0;
+  std::vector<HostTables> tables;
+  cel_physics phys{};
+  cel_geometry geo{};
+  std::vector<double> h_bounds; std::vector<int> h_vol_material, h_vol_bin;
+  uint64_t n_slots = 0;
+  // device-resident read-only data (small)
+  void* d_params_blob = nullptr;
+  // workspace
+  void* workspace = nullptr; uint64_t workspace_bytes = 0; bool own_workspace = false; bool laid_out = false;
+  // stream-ordered scratch of the current run
+  void* scratch = nullptr; void* d_tally = nullptr; void* d_prim = nullptr;
+  cudaStream_t stream = nullptr; bool own_stream = false;
+  cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
+  Control* h_status = nullptr;      // pinned, kStatusSlots entries
+  uint64_t* h_tally = nullptr; size_t h_tally_bytes = 0;   // pinned
+  void* h_prim = nullptr; size_t h_prim_bytes = 0;         // pinned staging of primaries
+  cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
+  int use_graph = 1; int batch = 16; int64_t max_iterations = 1ll << 22;
+  int n_sm = 148;
+  bool ran = false; int run_error = 0;
+  uint64_t launches = 0; int kernels_per_iteration = 0;
+  Control last{};                   // final status of the last run
+  std::string cuda_error;
+};
+
+namespace {
+
+#define CEL_CUDA(ctx, call)                                                        \
+  do {                                                                             \
+    cudaError_t e_ = (call);                                                       \
+    if (e_ != cudaSuccess) {                                                       \
+      (ctx)->cuda_error = std::string(#call) + ": " + cudaGetErrorString(e_);      \
+      return (e_ == cudaErrorMemoryAllocation) ? CEL_ERR_OOM : CEL_ERR_CUDA;       \
+    }                                                                              \
+  } while (0)
+
+inline uint64_t align_up(uint64_t x, uint64_t a) { return (x + a - 1) / a * a; }
+
+// ---------------------------------------------------------------- S4: physics tables, built on the host
+double klein_nishina_total(double E) {
+  const double k = E / kElectronMass;
+  const double L = std::log1p(2.0 * k);
+  const double a = (1.0 + k) / (k * k) * (2.0 * (1.0 + k) / (1.0 + 2.0 * k) - L / k);
+  const double b = L / (2.0 * k);
+  const double c = (1.0 + 3.0 * k) / ((1.0 + 2.0 * k) * (1.0 + 2.0 * k));
+  return 2.0 * kPi * kClassicalRadius * kClassicalRadius * (a + b - c);
+}
+
+struct MaterialHost { double n_atom, n_e, I, L_rad, inv_X0, Z; };
+
+double collision_stopping_power(const MaterialHost& m, double T) {
+  const double tau = T / kElectronMass;
+  const double g1 = tau + 1.0;
+  const double beta2 = tau * (tau + 2.0) / (g1 * g1);
+  const double ir = m.I / kElectronMass;
+  const double br = std::log(tau * tau * (tau + 2.0) / (2.0 * ir * ir)) + 1.0 - beta2 +
+                    (tau * tau / 8.0 - (2.0 * tau + 1.0) * std::log(2.0)) / (g1 * g1);
+  return 2.0 * kPi * kClassicalRadius * kClassicalRadius * kElectronMass * m.n_e / beta2 * br;
+}
+
+void build_tables(const cel_material& mat, const cel_physics& ph, HostTables& out) {
+  MaterialHost m;
+  m.Z = mat.Z;
+  m.n_atom = mat.density_g_cm3 * kAvogadro / mat.A;
+  m.n_e = mat.Z * m.n_atom;
+  m.I = 16e-6 * std::pow(mat.Z, 0.9);
+  m.L_rad = std::log(183.0 * std::pow(mat.Z, -1.0 / 3.0));
+  m.inv_X0 = 4.0 * kFineStructure * kClassicalRadius * kClassicalRadius * m.n_atom * mat.Z * (mat.Z + 1.0) * m.L_rad;
+  out.inv_X0 = m.inv_X0;
+  const double u0 = std::log(1e-3), du = std::log(10.0) / 64.0;
+  const double n_pb = 11.35 * kAvogadro / 207.2;
+  for (auto& v : out.t) v.assign(kGrid, 0.0);
+  for (int j = 0; j < kGrid; ++j) {
+    const double E = std::exp(u0 + j * du);
+    out.t[0][j] = m.n_e * klein_nishina_total(E);
+    out.t[1][j] = (m.n_atom / n_pb) * std::pow(mat.Z / 82.0, 5.0) * std::pow(E, -3.5);
+    const double no_screen = (28.0 / 9.0) * std::log(2.0 * E / kElectronMass) - 218.0 / 27.0;
+    const double full_screen = (28.0 / 9.0) * m.L_rad - 2.0 / 27.0;
+    const double f = std::fmax(0.0, std::fmin(no_screen, full_screen));
+    out.t[2][j] = ph.enable_pair ? m.n_atom * kFineStructure * kClassicalRadius * kClassicalRadius * mat.Z * (mat.Z + 1.0) * f : 0.0;
+    out.t[3][j] = ph.enable_brems ? std::fmax(0.0, std::log(E / ph.cut_MeV)) * m.inv_X0 : 0.0;
+  }
+  // range: composite Simpson in u = ln T, 64 sub-intervals per cell
+  out.t[4][0] = 0.0;
+  for (int j = 1; j < kGrid; ++j) {
+    const double lo = u0 + (j - 1) * du, hi = u0 + j * du;
+    const int n = 64;
+    const double h = (hi - lo) / n;
+    double acc = 0.0;
+    for (int i = 0; i <= n; ++i) {
+      const double T = std::exp(lo + i * h);
+      const double w = (i == 0 || i == n) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
+      acc += w * (T / collision_stopping_power(m, T));
+    }
+    out.t[4][j] = out.t[4][j - 1] + acc * h / 3.0;
+  }
+}
+
+int host_locate(const cel_geometry& g, const double* bounds, const double pos[3], const double dir[3]) {
+  if (g.kind == CEL_GEOM_SLAB) {
+    for (int i = 0; i < g.n_vol; ++i) {
+      const double lo = bounds[i], hi = bounds[i + 1];
+      if (pos[2] > lo && pos[2] < hi) return i;
+      if (pos[2] == lo && dir[2] >= 0.0) return i;
+      if (pos[2] == hi && dir[2] < 0.0) return i;
+    }
+    return -1;
+  }
+  const double r = std::sqrt(pos[0] * pos[0] + pos[1] * pos[1]);
+  for (int i = 0; i < g.n_vol; ++i)
+    if (r >= bounds[i] && r < bounds[i + 1]) return i;
+  return -1;
+}
+
+}  // namespace
+
+// ================================================================ workspace layout
+namespace {
+
+struct Layout {
+  uint64_t stA, stB, akey, nsec, indices, stage, secA, secB, initA, initB, ctl, log, total;
+};
+
+Layout make_layout(uint64_t N, uint64_t cap, int sort_mode) {
+  Layout L{};
+  const uint64_t tiles = (N + kTile - 1) / kTile;
+  uint64_t o = 0;
+  auto take = [&](uint64_t bytes) { uint64_t r = o; o = align_up(o + bytes, 256); return r; };
+  L.stA = take(N * sizeof(RecA));
+  L.stB = take(N * sizeof(RecB));
+  L.akey = take(tiles * kTile);
+  L.nsec = take(tiles * kTile);
+  L.indices = take(sort_mode != CEL_SORT_NONE ? N * sizeof(uint32_t) : 0);
+  L.stage = take(N * sizeof(Stage));
+  L.secA = take(2 * N * sizeof(RecA));
+  L.secB = take(2 * N * sizeof(RecB));
+  L.initA = take(cap * sizeof(RecA));
+  L.initB = take(cap * sizeof(RecB));
+  L.ctl = take(sizeof(Control));
+  L.log = take((uint64_t)kLogCapacity * 8 * sizeof(uint32_t));
+  L.total = o;
+  return L;
+}
+
+uint64_t default_capacity(uint64_t N, uint64_t cap) {
+  if (cap != 0) return cap;
+  const uint64_t c = 8 * N;
+  return c > (1ull << 24) ? c : (1ull << 24);
+}
+
+int lay_out(cel_ctx* c) {
+  if (c->laid_out) return CEL_OK;
+  const Layout L = make_layout(c->n_slots, c->D.init_capacity, c->D.sort_mode);
+  if (!c->workspace) {
+    CEL_CUDA(c, cudaMalloc(&c->workspace, L.total));
+    c->workspace_bytes = L.total; c->own_workspace = true;
+  } else if (c->workspace_bytes < L.total) {
+    return CEL_ERR_INVALID_ARG;
+  }
+  char* base = (char*)c->workspace;
+  DeviceState& D = c->D;
+  D.stA = (RecA*)(base + L.stA); D.stB = (RecB*)(base + L.stB);
+  D.akey = (uint8_t*)(base + L.akey); D.nsec = (uint8_t*)(base + L.nsec);
+  D.indices = (D.sort_mode != CEL_SORT_NONE) ? (uint32_t*)(base + L.indices) : nullptr;
+  D.stage = (Stage*)(base + L.stage);
+  D.secA = (RecA*)(base + L.secA); D.secB = (RecB*)(base + L.secB);
+  D.initA = (RecA*)(base + L.initA); D.initB = (RecB*)(base + L.initB);
+  D.ctl = (Control*)(base + L.ctl);
+  D.counts_log = (uint32_t*)(base + L.log);
+  D.log_capacity = kLogCapacity;
+  c->laid_out = true;
+  return CEL_OK;
+}
+
+}  // namespace
+
+extern "C" uint64_t cel_workspace_bytes(uint64_t n_slots, uint64_t init_capacity, int sort_mode) {
+  return make_layout(n_slots, default_capacity(n_slots, init_capacity), sort_mode).total;
+}
+
+// ================================================================ create / destroy
+extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n_mats, const cel_physics* ph,
+                          uint64_t n_slots, int sort_mode, cel_ctx** out) {
+  if (!g || !mats || !ph || !out || n_mats < 1 || n_slots < 1 || n_slots > (1ull << 31)) return CEL_ERR_INVALID_ARG;
+  if (sort_mode < 0 || sort_mode > 2 || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
+  if (g->n_vol < 1 || g->n_vol > 254 || !g->bounds || !g->vol_material || !g->vol_bin) return CEL_ERR_INVALID_ARG;
+  for (int i = 0; i < g->n_vol; ++i) {
+    if (!(g->bounds[i] < g->bounds[i + 1])) return CEL_ERR_INVALID_ARG;
+    if (g->vol_material[i] < -1 || g->vol_material[i] >= n_mats || g->vol_bin[i] < -1) return CEL_ERR_INVALID_ARG;
+  }
+  if (g->kind == CEL_GEOM_CYL && g->bounds[0] != 0.0) return CEL_ERR_INVALID_ARG;
+  if (!(ph->cut_MeV > 0.0) || ph->max_substeps < 1) return CEL_ERR_INVALID_ARG;
+  for (int i = 0; i < n_mats; ++i)
+    if (!(mats[i].density_g_cm3 > 0.0) || !(mats[i].Z > 0.0) || !(mats[i].A > 0.0)) return CEL_ERR_INVALID_ARG;
+
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) return CEL_ERR_CUDA;  // no CPU fallback
+
+  cel_ctx* c = new cel_ctx();
+  c->geo = *g; c->phys = *ph; c->n_mats = n_mats; c->n_slots = n_slots;
+  c->h_bounds.assign(g->bounds, g->bounds + g->n_vol + 1);
+  c->h_vol_material.assign(g->vol_material, g->vol_material + g->n_vol);
+  c->h_vol_bin.assign(g->vol_bin, g->vol_bin + g->n_vol);
+  c->geo.bounds = c->h_bounds.data(); c->geo.vol_material = c->h_vol_material.data(); c->geo.vol_bin = c->h_vol_bin.data();
+  c->tables.resize(n_mats);
+  for (int i = 0; i < n_mats; ++i) build_tables(mats[i], *ph, c->tables[i]);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+
+  // one blob with all read-only device data: bounds | vol_material | vol_bin | mats | photon_xs | charged_xs | range
+  const uint64_t o_bounds = 0;
+  const uint64_t o_vm = align_up(o_bounds + (g->n_vol + 1) * sizeof(double), 256);
+  const uint64_t o_vb = align_up(o_vm + g->n_vol * sizeof(int), 256);
+  const uint64_t o_mats = align_up(o_vb + g->n_vol * sizeof(int), 256);
+  const uint64_t o_ph = align_up(o_mats + n_mats * sizeof(MaterialDev), 256);
+  const uint64_t o_ch = align_up(o_ph + (uint64_t)n_mats * kGrid * sizeof(PhotonXs), 256);
+  const uint64_t o_rg = align_up(o_ch + (uint64_t)n_mats * kGrid * sizeof(ChargedXs), 256);
+  const uint64_t blob_bytes = align_up(o_rg + (uint64_t)n_mats * kGrid * sizeof(double), 256);
+  std::vector<char> blob(blob_bytes, 0);
+  std::memcpy(blob.data() + o_bounds, c->h_bounds.data(), (g->n_vol + 1) * sizeof(double));
+  std::memcpy(blob.data() + o_vm, c->h_vol_material.data(), g->n_vol * sizeof(int));
+  std::memcpy(blob.data() + o_vb, c->h_vol_bin.data(), g->n_vol * sizeof(int));
+  for (int m = 0; m < n_mats; ++m) {
+    ((MaterialDev*)(blob.data() + o_mats))[m].inv_X0 = c->tables[m].inv_X0;
+    for (int j = 0; j < kGrid; ++j) {
+      PhotonXs& px = ((PhotonXs*)(blob.data() + o_ph))[(size_t)m * kGrid + j];
+      px.compton = c->tables[m].t[0][j]; px.pe = c->tables[m].t[1][j]; px.pair = c->tables[m].t[2][j]; px.pad = 0.0;
+      ChargedXs& cx = ((ChargedXs*)(blob.data() + o_ch))[(size_t)m * kGrid + j];
+      cx.brems = c->tables[m].t[3][j]; cx.range = c->tables[m].t[4][j];
+      ((double*)(blob.data() + o_rg))[(size_t)m * kGrid + j] = c->tables[m].t[4][j];
+    }
+  }
+  auto fail = [&](int code) { cel_destroy(c); return code; };
+  if (cudaMalloc(&c->d_params_blob, blob_bytes) != cudaSuccess) return fail(CEL_ERR_OOM);
+  if (cudaMemcpy(c->d_params_blob, blob.data(), blob_bytes, cudaMemcpyHostToDevice) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  char* db = (char*)c->d_params_blob;
+
+  DeviceState& D = c->D;
+  Params& P = D.P;
+  P.geom_kind = g->kind; P.n_vol = g->n_vol;
+  int nb = 0;
+  for (int i = 0; i < g->n_vol; ++i) if (g->vol_bin[i] + 1 > nb) nb = g->vol_bin[i] + 1;
+  P.n_bins = nb;
+  P.bounds = (const double*)(db + o_bounds); P.vol_material = (const int*)(db + o_vm); P.vol_bin = (const int*)(db + o_vb);
+  P.half_x = g->half_x; P.half_y = g->half_y; P.half_z = g->half_z;
+  const double bm = std::sqrt(g->field_T[0] * g->field_T[0] + g->field_T[1] * g->field_T[1] + g->field_T[2] * g->field_T[2]);
+  P.bmag = bm;
+  P.bhx = bm > 0.0 ? g->field_T[0] / bm : 0.0; P.bhy = bm > 0.0 ? g->field_T[1] / bm : 0.0; P.bhz = bm > 0.0 ? g->field_T[2] / bm : 0.0;
+  P.key0 = (uint32_t)(ph->seed & 0xffffffffu); P.key1 = (uint32_t)(ph->seed >> 32);
+  P.cut = ph->cut_MeV;
+  P.enable_msc = ph->enable_msc; P.enable_eloss = ph->enable_eloss; P.enable_annihilation = ph->enable_annihilation;
+  P.electrons_local = ph->electrons_local; P.max_substeps = ph->max_substeps; P.max_steps_per_track = ph->max_steps_per_track;
+  P.u0 = std::log(1e-3); P.du = std::log(10.0) / 64.0; P.inv_du = 1.0 / P.du;
+  P.mats = (const MaterialDev*)(db + o_mats); P.photon_xs = (const PhotonXs*)(db + o_ph);
+  P.charged_xs = (const ChargedXs*)(db + o_ch); P.range_tab = (const double*)(db + o_rg);
+  D.N = (uint32_t)n_slots; D.n_tiles = (uint32_t)((n_slots + kTile - 1) / kTile);
+  D.sort_mode = sort_mode;
+  D.init_capacity = default_capacity(n_slots, ph->init_capacity);
+
+  if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  c->own_stream = true;
+  if (cudaEventCreate(&c->ev_start) != cudaSuccess || cudaEventCreate(&c->ev_stop) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  for (int i = 0; i < kStatusSlots; ++i)
+    if (cudaEventCreateWithFlags(&c->ev_batch[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  if (cudaMallocHost((void**)&c->h_status, kStatusSlots * sizeof(Control)) != cudaSuccess) return fail(CEL_ERR_OOM);
+  *out = c;
+  return CEL_OK;
+}
+
+extern "C" void cel_destroy(cel_ctx* c) {
+  if (!c) return;
+  if (c->stream) cudaStreamSynchronize(c->stream);
+  if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+  if (c->graph) cudaGraphDestroy(c->graph);
+  if (c->scratch) cudaFree(c->scratch);
+  if (c->d_tally) cudaFree(c->d_tally);
+  if (c->d_prim) cudaFree(c->d_prim);
+  if (c->own_workspace && c->workspace) cudaFree(c->workspace);
+  if (c->d_params_blob) cudaFree(c->d_params_blob);
+  if (c->h_status) cudaFreeHost(c->h_status);
+  if (c->h_tally) cudaFreeHost(c->h_tally);
+  if (c->h_prim) cudaFreeHost(c->h_prim);
+  if (c->ev_start) cudaEventDestroy(c->ev_start);
+  if (c->ev_stop) cudaEventDestroy(c->ev_stop);
+  for (int i = 0; i < kStatusSlots; ++i) if (c->ev_batch[i]) cudaEventDestroy(c->ev_batch[i]);
+  if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+  delete c;
+}
+
+extern "C" int cel_set_stream(cel_ctx* c, void* s) {
+  if (!c || c->ran) return CEL_ERR_INVALID_ARG;
+  if (c->own_stream && c->stream) { cudaStreamDestroy(c->stream); c->own_stream = false; }
+  c->stream = (cudaStream_t)s;
+  return CEL_OK;
+}
+
+extern "C" int cel_set_workspace(cel_ctx* c, void* dptr, uint64_t bytes) {
+  if (!c || !dptr || c->laid_out || ((uintptr_t)dptr & 255)) return CEL_ERR_INVALID_ARG;
+  if (bytes < make_layout(c->n_slots, c->D.init_capacity, c->D.sort_mode).total) return CEL_ERR_INVALID_ARG;
+  c->workspace = dptr; c->workspace_bytes = bytes; c->own_workspace = false;
+  return CEL_OK;
+}
+
+extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
+  if (!c || !name) return CEL_ERR_INVALID_ARG;
+  if (!std::strcmp(name, "use_graph")) c->use_graph = v ? 1 : 0;
+  else if (!std::strcmp(name, "batch")) { if (v < 1 || v > 4096) return CEL_ERR_INVALID_ARG; c->batch = (int)v; }
+  else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
+  else return CEL_ERR_INVALID_ARG;
+  return CEL_OK;
+}
+
+extern "C" const char* cel_strerror(int code) {
+  switch (code) {
+    case CEL_OK: return "ok";
+    case CEL_ERR_INVALID_ARG: return "invalid argument";
+    case CEL_ERR_CUDA: return "CUDA runtime error";
+    case CEL_ERR_OOM: return "out of memory";
+    case CEL_ERR_INIT_OVERFLOW: return "initializer stack overflow";
+    case CEL_ERR_TALLY_OVERFLOW: return "tally overflow";
+    case CEL_ERR_NONFINITE: return "non-finite track state";
+    case CEL_ERR_NOT_RUN: return "no transport has run";
+    case CEL_ERR_MAX_ITER: return "iteration limit reached";
+    default: return "unknown error";
+  }
+}
+extern "C" const char* cel_last_cuda_error(cel_ctx* c) { return c ? c->cuda_error.c_str() : ""; }
+
+// ================================================================ the step iteration and the host loop
+namespace {
+
+int physics_grid(const cel_ctx* c) {
+  const uint64_t need = (c->n_slots + kBlock - 1) / kBlock;
+  const uint64_t cap = (uint64_t)c->n_sm * 8;
+  return (int)(need < cap ? need : cap);
+}
+
+// one step iteration = P1, P2, P3i, P3m, P4, P5 (docs/PHYSICS_SPEC.md S1); returns the number of kernels enqueued
+int enqueue_iteration(cel_ctx* c) {
+  const DeviceState& D = c->D;
+  cudaStream_t s = c->stream;
+  const int tg = (int)D.n_tiles;
+  const int pg = physics_grid(c);
+  int n = 0;
+  k_vac_count<<<tg, kTileThreads, 0, s>>>(D); ++n;
+  k_init_fill<<<tg, kTileThreads, 0, s>>>(D); ++n;
+  if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); ++n; }
+  k_interact<A_PE><<<pg, kBlock, 0, s>>>(D); ++n;
+  if (c->phys.enable_pair) { k_interact<A_PAIR><<<pg, kBlock, 0, s>>>(D); ++n; }
+  k_interact<A_COMPTON><<<pg, kBlock, 0, s>>>(D); ++n;
+  if (c->phys.enable_brems) { k_interact<A_BREMS><<<pg, kBlock, 0, s>>>(D); ++n; }
+  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); ++n; }
+  k_move_photon<<<pg, kBlock, 0, s>>>(D); ++n;
+  k_move_charged<<<pg, kBlock, 0, s>>>(D); ++n;
+  k_score<<<pg, kBlock, 0, s>>>(D); ++n;
+  k_push_count<<<tg, kTileThreads, 0, s>>>(D); ++n;
+  k_push_write<<<tg, kTileThreads, 0, s>>>(D); ++n;
+  return n;
+}
+
+// reset slots, staging, counters and tallies; allocate the run's scratch with the stream-ordered allocator
+int prepare_run(cel_ctx* c, uint32_t n_events) {
+  int rc = lay_out(c);
+  if (rc != CEL_OK) return rc;
+  cudaStream_t s = c->stream;
+  DeviceState& D = c->D;
+  // stream-ordered scratch: freed and re-allocated on the stream, never a device-wide sync
+  if (c->scratch) { CEL_CUDA(c, cudaFreeAsync(c->scratch, s)); c->scratch = nullptr; }
+  if (c->d_tally) { CEL_CUDA(c, cudaFreeAsync(c->d_tally, s)); c->d_tally = nullptr; }
+  const uint64_t tiles = D.n_tiles;
+  const uint64_t o_vac = 0, o_hist = align_up(tiles * 4, 256), o_sec = align_up(o_hist + tiles * 32, 256);
+  const uint64_t scratch_bytes = align_up(o_sec + tiles * 4, 256);
+  CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
+  const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
+  CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));
+  D.tile_vac = (uint32_t*)((char*)c->scratch + o_vac);
+  D.tile_hist = (uint32_t*)((char*)c->scratch + o_hist);
+  D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
+  D.tally = (unsigned long long*)c->d_tally;
+  D.n_events = n_events;
+  CEL_CUDA(c, cudaMemsetAsync(c->scratch, 0, scratch_bytes, s));
+  CEL_CUDA(c, cudaMemsetAsync(c->d_tally, 0, tally_bytes > 0 ? tally_bytes : 8, s));
+  CEL_CUDA(c, cudaMemsetAsync(D.ctl, 0, sizeof(Control), s));
+  k_reset_state<<<c->n_sm * 4, 256, 0, s>>>(D);
+  CEL_CUDA(c, cudaGetLastError());
+  // pinned tally buffer for cel_tallies
+  if (c->h_tally_bytes < tally_bytes) {
+    if (c->h_tally) cudaFreeHost(c->h_tally);
+    c->h_tally = nullptr; c->h_tally_bytes = 0;
+    CEL_CUDA(c, cudaMallocHost((void**)&c->h_tally, tally_bytes));
+    c->h_tally_bytes = tally_bytes;
+  }
+  // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
+  if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+  if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+  if (c->use_graph) {
+    CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
+    c->kernels_per_iteration = enqueue_iteration(c);
+    CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
+    CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+  }
+  c->launches = 0; c->run_error = 0; c->ran = true;
+  std::memset(&c->last, 0, sizeof(Control));
+  return CEL_OK;
+}
+
+int validate_primaries(const cel_ctx* c, const cel_primary* p, uint64_t n, uint32_t n_events) {
+  for (uint64_t i = 0; i < n; ++i) {
+    if (p[i].event >= n_events || p[i].event >= (1u << 24) || p[i].ptype < 0 || p[i].ptype > 2) return CEL_ERR_INVALID_ARG;
+    if (!(p[i].energy_MeV > 0.0) || !std::isfinite(p[i].energy_MeV)) return CEL_ERR_INVALID_ARG;
+    const double* d = p[i].dir;
+    const double n2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    if (!(std::fabs(n2 - 1.0) <= 1e-12)) return CEL_ERR_INVALID_ARG;
+    if (host_locate(c->geo, c->h_bounds.data(), p[i].pos, p[i].dir) < 0) return CEL_ERR_INVALID_ARG;
+    if (c->geo.kind == CEL_GEOM_SLAB && (std::fabs(p[i].pos[0]) > c->geo.half_x || std::fabs(p[i].pos[1]) > c->geo.half_y)) return CEL_ERR_INVALID_ARG;
+    if (c->geo.kind == CEL_GEOM_CYL && std::fabs(p[i].pos[2]) > c->geo.half_z) return CEL_ERR_INVALID_ARG;
+  }
+  return CEL_OK;
+}
+
+// host primaries -> pinned staging -> device scratch (stream-ordered) -> init[i]
+int load_primaries_host(cel_ctx* c, const cel_primary* p, uint64_t n) {
+  cudaStream_t s = c->stream;
+  const size_t bytes = n * sizeof(cel_primary);
+  if (c->h_prim_bytes < bytes) {
+    if (c->h_prim) cudaFreeHost(c->h_prim);
+    c->h_prim = nullptr; c->h_prim_bytes = 0;
+    CEL_CUDA(c, cudaMallocHost(&c->h_prim, bytes));
+    c->h_prim_bytes = bytes;
+  }
+  if (n) std::memcpy(c->h_prim, p, bytes);
+  if (c->d_prim) { CEL_CUDA(c, cudaFreeAsync(c->d_prim, s)); c->d_prim = nullptr; }
+  CEL_CUDA(c, cudaMallocAsync(&c->d_prim, bytes ? bytes : 64, s));
+  if (n) CEL_CUDA(c, cudaMemcpyAsync(c->d_prim, c->h_prim, bytes, cudaMemcpyHostToDevice, s));
+  k_load_primaries<<<c->n_sm, 256, 0, s>>>(c->D, (const PrimaryRec*)c->d_prim, n);
+  CEL_CUDA(c, cudaGetLastError());
+  return CEL_OK;
+}
+
+// enqueue batches of iterations; after each batch copy the control block to pinned memory asynchronously and look
+// at the PREVIOUS batch's copy, so the device always has a batch queued while the host decides
+int run_loop(cel_ctx* c) {
+  cudaStream_t s = c->stream;
+  CEL_CUDA(c, cudaEventRecord(c->ev_start, s));
+  int64_t enqueued = 0;
+  int slot = 0;
+  bool have_prev = false;
+  int rc = CEL_OK;
+  while (true) {
+    for (int b = 0; b < c->batch; ++b) {
+      if (c->use_graph) { CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s)); c->launches += c->kernels_per_iteration; }
+      else c->launches += enqueue_iteration(c);
+    }
+    enqueued += c->batch;
+    CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
+    CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
+    if (have_prev) {
+      const int prev = slot ^ 1;
+      CEL_CUDA(c, cudaEventSynchronize(c->ev_batch[prev]));
+      const Control& st = c->h_status[prev];
+      if (st.error != 0) { rc = st.error; break; }
+      if (st.finished) break;
+    }
+    if (enqueued >= c->max_iterations) { rc = CEL_ERR_MAX_ITER; break; }
+    have_prev = true;
+    slot ^= 1;
+  }
+  CEL_CUDA(c, cudaGetLastError());
+  CEL_CUDA(c, cudaEventRecord(c->ev_stop, s));
+  c->run_error = rc;
+  return rc;
+}
+
+}  // namespace
+
+extern "C" int cel_transport(cel_ctx* c, const cel_primary* primaries, uint64_t n, uint32_t n_events) {
+  if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  int rc = validate_primaries(c, primaries, n, n_events);
+  if (rc != CEL_OK) return rc;
+  if ((rc = prepare_run(c, n_events)) != CEL_OK) return rc;
+  if ((rc = load_primaries_host(c, primaries, n)) != CEL_OK) return rc;
+  return run_loop(c);
+}
+
+extern "C" int cel_transport_device(cel_ctx* c, const void* d_primaries, uint64_t n, uint32_t n_events) {
+  if (!c || (!d_primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  int rc = prepare_run(c, n_events);
+  if (rc != CEL_OK) return rc;
+  k_load_primaries<<<c->n_sm, 256, 0, c->stream>>>(c->D, (const PrimaryRec*)d_primaries, n);
+  CEL_CUDA(c, cudaGetLastError());
+  return run_loop(c);
+}
+
+extern "C" int cel_tallies(cel_ctx* c, cel_tally_view* out) {
+  if (!c || !out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  cudaStream_t s = c->stream;
+  const DeviceState& D = c->D;
+  const uint64_t bytes = (uint64_t)D.n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
+  CEL_CUDA(c, cudaMemcpyAsync(c->h_tally, D.tally, bytes, cudaMemcpyDeviceToHost, s));
+  CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[0], D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
+  CEL_CUDA(c, cudaStreamSynchronize(s));
+  c->last = c->h_status[0];
+  out->n_events = D.n_events; out->n_bins = D.P.n_bins; out->fixed = c->h_tally;
+  out->track_steps = c->last.track_steps; out->iterations = c->last.iterations; out->secondaries = c->last.secondaries;
+  float ms = 0.f;
+  out->seconds = (cudaEventElapsedTime(&ms, c->ev_start, c->ev_stop) == cudaSuccess) ? ms * 1e-3 : 0.0;
+  out->kernel_launches = c->launches;
+  if (c->last.error != 0) return c->last.error;
+  return c->run_error;
+}
+
+// ================================================================ debug / parity surface (synchronous)
+extern "C" int cel_debug_begin(cel_ctx* c, const cel_primary* primaries, uint64_t n, uint32_t n_events) {
+  if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  int rc = validate_primaries(c, primaries, n, n_events);
+  if (rc != CEL_OK) return rc;
+  if ((rc = prepare_run(c, n_events)) != CEL_OK) return rc;
+  if ((rc = load_primaries_host(c, primaries, n)) != CEL_OK) return rc;
+  CEL_CUDA(c, cudaEventRecord(c->ev_start, c->stream));
+  CEL_CUDA(c, cudaEventRecord(c->ev_stop, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  return CEL_OK;
+}
+
+extern "C" int cel_debug_step(cel_ctx* c) {
+  if (!c || !c->ran) return CEL_ERR_NOT_RUN;
+  c->launches += enqueue_iteration(c);
+  CEL_CUDA(c, cudaGetLastError());
+  CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[0], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->last = c->h_status[0];
+  return c->last.error;
+}
+
+namespace {
+int unpack_to_host(cel_ctx* c, const RecA* A, const RecB* B, uint64_t n, int as_init, cel_track* host_out) {
+  if (n == 0) return CEL_OK;
+  void* d = nullptr;
+  CEL_CUDA(c, cudaMallocAsync(&d, n * sizeof(TrackRec), c->stream));
+  k_unpack<<<c->n_sm * 2, 256, 0, c->stream>>>(A, B, (TrackRec*)d, n, as_init);
+  CEL_CUDA(c, cudaGetLastError());
+  CEL_CUDA(c, cudaMemcpyAsync(host_out, d, n * sizeof(TrackRec), cudaMemcpyDeviceToHost, c->stream));
+  CEL_CUDA(c, cudaFreeAsync(d, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  return CEL_OK;
+}
+int fetch_control(cel_ctx* c) {
+  CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[0], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  c->last = c->h_status[0];
+  return CEL_OK;
+}
+}  // namespace
+
+extern "C" int cel_debug_read_state(cel_ctx* c, cel_track* host_out) {
+  if (!c || !host_out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  return unpack_to_host(c, c->D.stA, c->D.stB, c->n_slots, 0, host_out);
+}
+
+extern "C" int cel_debug_read_indices(cel_ctx* c, uint32_t* idx, uint32_t* offsets) {
+  if (!c || !idx || !offsets) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  int rc = fetch_control(c);
+  if (rc != CEL_OK) return rc;
+  std::memcpy(offsets, c->last.offsets, 9 * sizeof(uint32_t));
+  if (c->D.sort_mode == CEL_SORT_NONE) {
+    for (uint64_t i = 0; i < c->n_slots; ++i) idx[i] = (uint32_t)i;
+  } else {
+    CEL_CUDA(c, cudaMemcpyAsync(idx, c->D.indices, c->n_slots * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return CEL_OK;
+}
+
+extern "C" int cel_debug_n_initializers(cel_ctx* c, uint64_t* n) {
+  if (!c || !n) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  int rc = fetch_control(c);
+  *n = c->last.n_init;
+  return rc;
+}
+
+extern "C" int cel_debug_read_initializers(cel_ctx* c, cel_track* host_out) {
+  if (!c || !host_out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  int rc = fetch_control(c);
+  if (rc != CEL_OK) return rc;
+  return unpack_to_host(c, c->D.initA, c->D.initB, c->last.n_init, 1, host_out);
+}
+
+extern "C" int cel_debug_n_counts(cel_ctx* c, uint64_t* n) {
+  if (!c || !n) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  int rc = fetch_control(c);
+  *n = c->last.n_logged;
+  return rc;
+}
+
+extern "C" int cel_debug_read_counts(cel_ctx* c, uint32_t* host_out) {
+  if (!c || !host_out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  int rc = fetch_control(c);
+  if (rc != CEL_OK) return rc;
+  if (c->last.n_logged) {
+    CEL_CUDA(c, cudaMemcpyAsync(host_out, c->D.counts_log, (uint64_t)c->last.n_logged * 8 * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  }
+  return CEL_OK;
+}
+
+extern "C" int cel_debug_table(cel_ctx* c, int material, int which, double* out577) {
+  if (!c || !out577 || material < 0 || material >= c->n_mats || which < 0 || which > 4) return CEL_ERR_INVALID_ARG;
+  // read back what the kernels actually use (device copy), not the host vector
+  const Params& P = c->D.P;
+  std::vector<double> tmp;
+  if (which <= 2) {
+    std::vector<PhotonXs> px(kGrid);
+    CEL_CUDA(c, cudaMemcpy(px.data(), P.photon_xs + (size_t)material * kGrid, kGrid * sizeof(PhotonXs), cudaMemcpyDeviceToHost));
+    for (int j = 0; j < kGrid; ++j) out577[j] = which == 0 ? px[j].compton : (which == 1 ? px[j].pe : px[j].pair);
+  } else if (which == 3) {
+    std::vector<ChargedXs> cx(kGrid);
+    CEL_CUDA(c, cudaMemcpy(cx.data(), P.charged_xs + (size_t)material * kGrid, kGrid * sizeof(ChargedXs), cudaMemcpyDeviceToHost));
+    for (int j = 0; j < kGrid; ++j) out577[j] = cx[j].brems;
+  } else {
+    CEL_CUDA(c, cudaMemcpy(out577, P.range_tab + (size_t)material * kGrid, kGrid * sizeof(double), cudaMemcpyDeviceToHost));
+  }
+  return CEL_OK;
+}
+
+extern "C" int cel_debug_uniforms(cel_ctx* c, const uint32_t* slots, uint32_t n, uint32_t k, uint32_t phase, uint32_t j, double* host_out) {
+  if (!c || !slots || !host_out) return CEL_ERR_INVALID_ARG;
+  if (n == 0) return CEL_OK;
+  void* ds = nullptr; void* dout = nullptr;
+  CEL_CUDA(c, cudaMallocAsync(&ds, n * sizeof(uint32_t), c->stream));
+  CEL_CUDA(c, cudaMallocAsync(&dout, n * sizeof(double), c->stream));
+  CEL_CUDA(c, cudaMemcpyAsync(ds, slots, n * sizeof(uint32_t), cudaMemcpyHostToDevice, c->stream));
+  k_debug_uniforms<<<(n + 255) / 256, 256, 0, c->stream>>>(c->D.P, (const uint32_t*)ds, n, k, phase, j, (double*)dout);
+  CEL_CUDA(c, cudaGetLastError());
+  CEL_CUDA(c, cudaMemcpyAsync(host_out, dout, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CEL_CUDA(c, cudaFreeAsync(ds, c->stream));
+  CEL_CUDA(c, cudaFreeAsync(dout, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  return CEL_OK;
+}

@@ -1,0 +1,272 @@
+// cel_device.cuh — device-side data layout and physics primitives of the celstep CUDA path (sm_100a).
+// Implements docs/PHYSICS_SPEC.md S0-S8 independently of the CPU oracle (no shared code or headers).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace cel {
+
+// ---------------------------------------------------------------- S0 constants
+constexpr double kElectronMass = 0.51099895;
+constexpr double kClassicalRadius = 2.8179403262e-13;
+constexpr double kAvogadro = 6.02214076e23;
+constexpr double kFineStructure = 7.2973525693e-3;
+constexpr double kKappa = 2.99792458;
+constexpr double kAlphaR = 0.2;
+constexpr double kRhoF = 0.01;
+constexpr double kDeltaChord = 1e-3;
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kTallyScale = 68719476736.0;  // 2^36
+constexpr int kGrid = 577;
+
+enum : int { A_PE = 0, A_PAIR = 1, A_COMPTON = 2, A_MOVE_G = 3, A_MOVE_C = 4, A_BREMS = 5, A_ANNIH = 6, A_VACANT = 7 };
+enum : int { P_GAMMA = 0, P_ELECTRON = 1, P_POSITRON = 2 };
+enum : uint32_t { PH_INTERACT = 0, PH_STEP = 1, PH_MSC = 2 };
+
+// ---------------------------------------------------------------- HBM layout
+// A slot's state is two 32-byte, 32-byte-aligned records, so that a gathered slot costs exactly two
+// sectors read and two written (the +344 % memory operations of PAPER.md:47 are sector amplification
+// of a field-per-array SoA under the index indirection).
+struct __align__(32) RecA { double x, y, z, energy; };
+struct __align__(32) RecB { double dx, dy, dz; unsigned long long meta; };
+// meta: bits 0-3 action | 4-5 ptype | 6 staged | 8-15 vol | 16-23 surf (0xff = none) | 24-39 nsteps | 40-63 event
+struct __align__(32) Stage { long long q_dep, q_esc; uint32_t event; int32_t bin; unsigned long long pad; };
+
+__device__ __forceinline__ int meta_action(unsigned long long m) { return (int)(m & 0xfull); }
+__device__ __forceinline__ int meta_ptype(unsigned long long m) { return (int)((m >> 4) & 0x3ull); }
+__device__ __forceinline__ bool meta_staged(unsigned long long m) { return (m >> 6) & 1ull; }
+__device__ __forceinline__ int meta_vol(unsigned long long m) { return (int)((m >> 8) & 0xffull); }
+__device__ __forceinline__ int meta_surf(unsigned long long m) { int s = (int)((m >> 16) & 0xffull); return s == 0xff ? -1 : s; }
+__device__ __forceinline__ uint32_t meta_nsteps(unsigned long long m) { return (uint32_t)((m >> 24) & 0xffffull); }
+__device__ __forceinline__ uint32_t meta_event(unsigned long long m) { return (uint32_t)(m >> 40); }
+__host__ __device__ __forceinline__ unsigned long long make_meta(int action, int ptype, bool staged, int vol, int surf,
+                                                                 uint32_t nsteps, uint32_t event) {
+  return (unsigned long long)(action & 0xf) | ((unsigned long long)(ptype & 0x3) << 4) | ((unsigned long long)(staged ? 1 : 0) << 6) |
+         ((unsigned long long)(vol & 0xff) << 8) | ((unsigned long long)((surf < 0 ? 0xff : surf) & 0xff) << 16) |
+         ((unsigned long long)(nsteps & 0xffff) << 24) | ((unsigned long long)event << 40);
+}
+// the dense key byte read by the scans: low nibble action, bits 4-5 particle type
+__host__ __device__ __forceinline__ uint8_t make_key(int action, int ptype) { return (uint8_t)((action & 0xf) | ((ptype & 0x3) << 4)); }
+
+// 256-bit global loads/stores (sm_100: LDG.E.256 / STG.E.256)
+__device__ __forceinline__ RecA load_a(const RecA* p) {
+  RecA r;
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(r.x), "=d"(r.y), "=d"(r.z), "=d"(r.energy) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void store_a(RecA* p, const RecA& r) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(r.x), "d"(r.y), "d"(r.z), "d"(r.energy) : "memory");
+}
+__device__ __forceinline__ RecB load_b(const RecB* p) {
+  long long a, b, c; unsigned long long m;
+  asm volatile("ld.global.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(m) : "l"(p));
+  RecB r; r.dx = __longlong_as_double(a); r.dy = __longlong_as_double(b); r.dz = __longlong_as_double(c); r.meta = m;
+  return r;
+}
+__device__ __forceinline__ void store_b(RecB* p, const RecB& r) {
+  asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(__double_as_longlong(r.dx)), "l"(__double_as_longlong(r.dy)),
+               "l"(__double_as_longlong(r.dz)), "l"(r.meta) : "memory");
+}
+__device__ __forceinline__ Stage load_stage(const Stage* p) {
+  Stage s; unsigned long long w2;
+  asm volatile("ld.global.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(s.q_dep), "=l"(s.q_esc), "=l"(w2), "=l"(s.pad) : "l"(p));
+  s.event = (uint32_t)w2; s.bin = (int32_t)(w2 >> 32);
+  return s;
+}
+__device__ __forceinline__ void store_stage(Stage* p, long long q_dep, long long q_esc, uint32_t event, int32_t bin) {
+  unsigned long long w2 = (unsigned long long)event | ((unsigned long long)(uint32_t)bin << 32);
+  asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(q_dep), "l"(q_esc), "l"(w2), "l"(0ull) : "memory");
+}
+
+// ---------------------------------------------------------------- per-context read-only device data
+struct MaterialDev { double inv_X0; };
+struct PhotonXs { double compton, pe, pair, pad; };   // one grid node, 32 B
+struct ChargedXs { double brems, range; };            // one grid node, 16 B
+
+struct Params {
+  // geometry
+  int geom_kind, n_vol, n_bins;
+  const double* bounds;        // n_vol+1
+  const int* vol_material;     // n_vol
+  const int* vol_bin;          // n_vol
+  double half_x, half_y, half_z;
+  double bmag, bhx, bhy, bhz;
+  // physics
+  uint32_t key0, key1;
+  double cut;
+  int enable_msc, enable_eloss, enable_annihilation, electrons_local, max_substeps;
+  uint32_t max_steps_per_track;
+  double u0, inv_du, du;
+  const MaterialDev* mats;
+  const PhotonXs* photon_xs;   // [n_mats][kGrid]
+  const ChargedXs* charged_xs; // [n_mats][kGrid]
+  const double* range_tab;     // [n_mats][kGrid]
+};
+
+// ---------------------------------------------------------------- S3 Philox4x32-10
+struct Philox4 { uint32_t w[4]; };
+
+__device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  Philox4 o; o.w[0] = c0; o.w[1] = c1; o.w[2] = c2; o.w[3] = c3;
+  return o;
+}
+__device__ __forceinline__ double to_uniform(uint32_t lo, uint32_t hi) {
+  unsigned long long x = ((unsigned long long)hi << 32) | lo;
+  return ((double)(x >> 12) + 0.5) * (1.0 / 4503599627370496.0);
+}
+// the two draws (2b, 2b+1) of block b of a phase
+__device__ __forceinline__ void draw_pair(const Params& P, uint32_t slot, uint32_t k, uint32_t phase, uint32_t block, double& xa, double& xb) {
+  Philox4 o = philox4x32_10(slot, k, phase, block, P.key0, P.key1);
+  xa = to_uniform(o.w[0], o.w[1]);
+  xb = to_uniform(o.w[2], o.w[3]);
+}
+
+// ---------------------------------------------------------------- S4 table lookups
+struct GridPos { int j; double f; };
+__device__ __forceinline__ GridPos grid_locate(const Params& P, double E) {
+  double t = (log(E) - P.u0) / P.du;
+  double fl = floor(t);
+  int j = fl < 0.0 ? 0 : (fl > 575.0 ? 575 : (int)fl);
+  GridPos g; g.j = j; g.f = t - (double)j;
+  return g;
+}
+__device__ __forceinline__ double lerp_node(double y0, double y1, double f) { return y0 + f * (y1 - y0); }
+
+// Rinv(r): largest j <= 575 with R_j <= r, scanning down from j_hint (the cell of the pre-step energy; r <= R(T0))
+__device__ __forceinline__ double range_inverse(const Params& P, const double* __restrict__ R, double r, int j_hint) {
+  int j = j_hint;
+  while (j > 0 && __ldg(R + j) > r) --j;
+  double Rj = __ldg(R + j), Rj1 = __ldg(R + j + 1);
+  double u = P.u0 + j * P.du + P.du * (r - Rj) / (Rj1 - Rj);
+  return exp(u);
+}
+
+// ---------------------------------------------------------------- vectors
+__device__ __forceinline__ void normalise3(double& x, double& y, double& z) {
+  double n = sqrt(x * x + y * y + z * z);
+  x /= n; y /= n; z /= n;
+}
+
+// S8 rotate(d, theta, phi) taking cos(theta), sin(theta)
+__device__ __forceinline__ void rotate_dir(double& dx, double& dy, double& dz, double ct, double st, double phi) {
+  double sp, cp;
+  sincos(phi, &sp, &cp);
+  double srho = sqrt(dx * dx + dy * dy);
+  double ox, oy, oz;
+  if (srho == 0.0) {
+    double sg = dz < 0.0 ? -1.0 : 1.0;
+    ox = st * cp; oy = st * sp; oz = sg * ct;
+  } else {
+    ox = dx * ct + st * (dx * dz * cp - dy * sp) / srho;
+    oy = dy * ct + st * (dy * dz * cp + dx * sp) / srho;
+    oz = dz * ct - srho * st * cp;
+  }
+  normalise3(ox, oy, oz);
+  dx = ox; dy = oy; dz = oz;
+}
+
+// ---------------------------------------------------------------- S6 geometry
+enum : int { HIT_Z = 1, HIT_X = 2, HIT_Y = 3, HIT_INNER = 4, HIT_OUTER = 5 };
+#define CEL_INF (__longlong_as_double(0x7ff0000000000000LL))
+
+__device__ __forceinline__ double clamp0(double s) { return s < 0.0 ? 0.0 : s; }
+
+__device__ __forceinline__ double distance_to_boundary(const Params& P, double x, double y, double z, double dx, double dy, double dz,
+                                                       int vol, int surf, int& which) {
+  if (P.geom_kind == 0) {
+    double sz = CEL_INF, sx = CEL_INF, sy = CEL_INF;
+    if (dz > 0.0) sz = clamp0((__ldg(P.bounds + vol + 1) - z) / dz);
+    else if (dz < 0.0) sz = clamp0((__ldg(P.bounds + vol) - z) / dz);
+    if (dx > 0.0) sx = clamp0((P.half_x - x) / dx);
+    else if (dx < 0.0) sx = clamp0((-P.half_x - x) / dx);
+    if (dy > 0.0) sy = clamp0((P.half_y - y) / dy);
+    else if (dy < 0.0) sy = clamp0((-P.half_y - y) / dy);
+    if (sz <= sx && sz <= sy) { which = HIT_Z; return sz; }
+    if (sx <= sy) { which = HIT_X; return sx; }
+    which = HIT_Y; return sy;
+  }
+  double a = dx * dx + dy * dy;
+  double b = x * dx + y * dy;
+  double r2 = x * x + y * y;
+  double s_in = CEL_INF, s_out = CEL_INF, s_z = CEL_INF;
+  if (a != 0.0) {
+    {
+      double rho = __ldg(P.bounds + vol + 1);
+      if (surf == vol + 1) {
+        s_out = (b >= 0.0) ? 0.0 : -2.0 * b / a;
+      } else {
+        double c = r2 - rho * rho;
+        double D = b * b - a * c;
+        if (D < 0.0) D = 0.0;
+        s_out = (b > 0.0) ? -c / (b + sqrt(D)) : (-b + sqrt(D)) / a;
+      }
+      s_out = clamp0(s_out);
+    }
+    if (vol > 0) {
+      double rho = __ldg(P.bounds + vol);
+      if (surf == vol) {
+        if (b < 0.0) s_in = 0.0;
+      } else if (b < 0.0) {
+        double c = r2 - rho * rho;
+        double D = b * b - a * c;
+        if (D > 0.0) s_in = clamp0(c / (-b + sqrt(D)));
+      }
+    }
+  }
+  if (dz > 0.0) s_z = clamp0((P.half_z - z) / dz);
+  else if (dz < 0.0) s_z = clamp0((-P.half_z - z) / dz);
+  if (s_in <= s_out && s_in <= s_z) { which = HIT_INNER; return s_in; }
+  if (s_out <= s_z) { which = HIT_OUTER; return s_out; }
+  which = HIT_Z; return s_z;
+}
+
+// apply the crossing; dz_sign is the z component of the direction of travel; returns true if escaped
+__device__ __forceinline__ bool cross_boundary(const Params& P, double& z, double dz_travel, int& vol, int& surf, int which) {
+  if (P.geom_kind == 0) {
+    surf = -1;
+    if (which != HIT_Z) return true;
+    if (dz_travel > 0.0) { z = __ldg(P.bounds + vol + 1); vol += 1; }
+    else { z = __ldg(P.bounds + vol); vol -= 1; }
+    return vol < 0 || vol >= P.n_vol;
+  }
+  if (which == HIT_Z) { surf = -1; return true; }
+  if (which == HIT_OUTER) { surf = vol + 1; vol += 1; return vol >= P.n_vol; }
+  surf = vol; vol -= 1;
+  return false;
+}
+
+// ---------------------------------------------------------------- S7.3 helix point after arc length h
+struct HelixFrame { double dpar, px, py, pz, wx, wy, wz; };  // d_par, d_perp, w = d x bh
+__device__ __forceinline__ HelixFrame helix_frame(const Params& P, double dx, double dy, double dz) {
+  HelixFrame F;
+  F.dpar = dx * P.bhx + dy * P.bhy + dz * P.bhz;
+  F.px = dx - F.dpar * P.bhx; F.py = dy - F.dpar * P.bhy; F.pz = dz - F.dpar * P.bhz;
+  F.wx = dy * P.bhz - dz * P.bhy; F.wy = dz * P.bhx - dx * P.bhz; F.wz = dx * P.bhy - dy * P.bhx;
+  return F;
+}
+__device__ __forceinline__ void helix_point(const Params& P, const HelixFrame& F, double x, double y, double z, double omega, double h,
+                                            double& ox, double& oy, double& oz, double& odx, double& ody, double& odz) {
+  double sn, cs;
+  sincos(omega * h, &sn, &cs);
+  double sh = sin(0.5 * omega * h);
+  double A = sn / omega;
+  double Bc = 2.0 * sh * sh / omega;
+  odx = F.dpar * P.bhx + cs * F.px + sn * F.wx;
+  ody = F.dpar * P.bhy + cs * F.py + sn * F.wy;
+  odz = F.dpar * P.bhz + cs * F.pz + sn * F.wz;
+  ox = x + h * F.dpar * P.bhx + A * F.px + Bc * F.wx;
+  oy = y + h * F.dpar * P.bhy + A * F.py + Bc * F.wy;
+  oz = z + h * F.dpar * P.bhz + A * F.pz + Bc * F.wz;
+}
+
+__device__ __forceinline__ long long quantise(double x) { return __double2ll_rn(x * kTallyScale); }
+
+}  // namespace cel
