@@ -474,11 +474,11 @@ __global__ void __launch_bounds__(kBlock) k_move_photon(DeviceState D) {
     double sPE = 0.0, sPair = 0.0, sC = 0.0;
     if (mat >= 0) {
       const GridPos g = grid_locate(P, a.energy);
-      const double4* xs = reinterpret_cast<const double4*>(P.photon_xs + (size_t)mat * kGrid + g.j);
-      const double4 n0 = __ldg(xs), n1 = __ldg(xs + 1);
-      sC = lerp_node(n0.x, n1.x, g.f);
-      sPE = lerp_node(n0.y, n1.y, g.f);
-      sPair = lerp_node(n0.z, n1.z, g.f);
+      const double2* xs = reinterpret_cast<const double2*>(P.photon_xs + (size_t)mat * kGrid + g.j);  // nodes j, j+1: 64 B
+      const double2 n0a = __ldg(xs), n0b = __ldg(xs + 1), n1a = __ldg(xs + 2), n1b = __ldg(xs + 3);
+      sC = lerp_node(n0a.x, n1a.x, g.f);
+      sPE = lerp_node(n0a.y, n1a.y, g.f);
+      sPair = lerp_node(n0b.x, n1b.x, g.f);
     }
     const double stot = (sPE + sPair) + sC;
     double xi0, xi1;
