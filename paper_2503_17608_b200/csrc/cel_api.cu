@@ -326,6 +326,8 @@ extern "C" int cel_set_stream(cel_ctx* c, void* s) {
   if (!c || c->ran) return CEL_ERR_INVALID_ARG;
   if (c->own_stream && c->stream) { cudaStreamDestroy(c->stream); c->own_stream = false; }
   c->stream = (cudaStream_t)s;
+  // the legacy default stream cannot be captured into a CUDA graph: launch the kernels directly there
+  if (c->stream == nullptr || c->stream == cudaStreamLegacy) c->use_graph = 0;
   return CEL_OK;
 }
 
@@ -380,11 +382,13 @@ int enqueue_iteration(cel_ctx* c) {
   k_vac_count<<<tg, kTileThreads, 0, s>>>(D); ++n;
   k_init_fill<<<tg, kTileThreads, 0, s>>>(D); ++n;
   if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); ++n; }
+  // ANNIH runs first: in the masked modes a positron stopped by the brems kernel of this iteration must not be
+  // picked up by the annihilation kernel until the next iteration (S1)
+  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); ++n; }
   k_interact<A_PE><<<pg, kBlock, 0, s>>>(D); ++n;
   if (c->phys.enable_pair) { k_interact<A_PAIR><<<pg, kBlock, 0, s>>>(D); ++n; }
   k_interact<A_COMPTON><<<pg, kBlock, 0, s>>>(D); ++n;
   if (c->phys.enable_brems) { k_interact<A_BREMS><<<pg, kBlock, 0, s>>>(D); ++n; }
-  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); ++n; }
   k_move_photon<<<pg, kBlock, 0, s>>>(D); ++n;
   k_move_charged<<<pg, kBlock, 0, s>>>(D); ++n;
   k_score<<<pg, kBlock, 0, s>>>(D); ++n;
