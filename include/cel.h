@@ -118,8 +118,22 @@ void cel_destroy(cel_ctx*);
 const char* cel_strerror(int code);
 const char* cel_last_cuda_error(cel_ctx*);
 
+/* The kernels of one step iteration, in launch order (S1). P1: VAC_COUNT, INIT_FILL; P2: SCATTER (sorted modes);
+ * P3i: ANNIH, PE, PAIR, COMPTON, BREMS; P3m: MOVE_G, MOVE_C; P4: SCORE; P5: PUSH_COUNT, PUSH_WRITE. */
+enum { CEL_K_VAC_COUNT = 0, CEL_K_INIT_FILL, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_COMPTON,
+       CEL_K_BREMS, CEL_K_MOVE_G, CEL_K_MOVE_C, CEL_K_SCORE, CEL_K_PUSH_COUNT, CEL_K_PUSH_WRITE, CEL_KERNEL_COUNT };
+int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
+const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
+/* Per-kernel device time of the last transport run with option "profile" = 1 (per-kernel HBM
+ * fractions). ms_out and launches_out are HOST arrays of CEL_KERNEL_COUNT entries: summed CUDA-event time between
+ * the launch before and the launch after each kernel on the context's stream, and the number of launches timed.
+ * All zero if the run was not profiled. */
+int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
+
 /* Run-time knobs (before a transport). use_graph: replay one captured CUDA graph per iteration (default 1).
- * batch: iterations enqueued between status polls (default 16). max_iterations: safety stop (default 2^22). */
+ * batch: iterations enqueued between status polls (default 16). max_iterations: safety stop (default 2^22).
+ * profile: 1 = launch the kernels directly with a CUDA event after each one and synchronise once per batch, so that
+ * cel_kernel_times can report per-kernel device time (a measurement mode: results are identical, the run is slower). */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* ---- debug / parity surface (synchronous, not timed) ---- */

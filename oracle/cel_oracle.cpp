@@ -39,6 +39,7 @@ const double KAPPA = 2.99792458;
 const double ALPHA_R = 0.2;
 const double RHO_F = 0.01;
 const double DELTA_CHORD = 1e-3;
+const int MAX_DIP_HALVINGS = 30;   // S7.3 dip rule
 const double PI = 3.14159265358979323846;
 const double INF = std::numeric_limits<double>::infinity();
 const double TALLY_SCALE = 68719476736.0;  // 2^36
@@ -278,6 +279,18 @@ double distance_to_boundary(const Geometry& g, const double pos[3], const double
   if (s_in <= s_out && s_in <= s_z) { *which = HIT_INNER; return s_in; }
   if (s_out <= s_z) { *which = HIT_OUTER; return s_out; }
   *which = HIT_Z; return s_z;
+}
+
+// S7.3 dip rule: does the tangent d point INTO the current volume across the surface that the chord ch hits?
+// (outward normal of the hit surface: the sign of the chord component for planes, radial for cylinders)
+bool tangent_points_inward(const Geometry& g, const double pos[3], const double d[3], const double ch[3], int which) {
+  if (g.kind == 0) {
+    const int axis = (which == HIT_Z) ? 2 : ((which == HIT_X) ? 0 : 1);
+    return d[axis] * ch[axis] < 0.0;
+  }
+  if (which == HIT_Z) return d[2] * ch[2] < 0.0;
+  const double radial = pos[0] * d[0] + pos[1] * d[1];
+  return (which == HIT_OUTER) ? (radial < 0.0) : (radial > 0.0);
 }
 
 // apply the crossing of surface `which`; returns true if the track escaped
@@ -605,13 +618,19 @@ void move_charged(Oracle& o, uint32_t slot) {
     while (!complete) {
       if (n == o.phys.max_substeps) break;  // paused
       double h = std::fmin(remaining, h_max);
-      double pn[3], dn[3];
-      helix_point(t.pos, t.dir, o.bh, omega, h, pn, dn);
-      double c[3] = {pn[0] - t.pos[0], pn[1] - t.pos[1], pn[2] - t.pos[2]};
-      double l = std::sqrt(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
-      double ch[3] = {c[0] / l, c[1] / l, c[2] / l};
+      double pn[3], dn[3], ch[3], l, tb;
       int which;
-      double tb = distance_to_boundary(o.geo, t.pos, ch, t.vol, t.surf, &which);
+      for (int halvings = 0;; ++halvings) {
+        helix_point(t.pos, t.dir, o.bh, omega, h, pn, dn);
+        double c[3] = {pn[0] - t.pos[0], pn[1] - t.pos[1], pn[2] - t.pos[2]};
+        l = std::sqrt(c[0] * c[0] + c[1] * c[1] + c[2] * c[2]);
+        for (int i = 0; i < 3; ++i) ch[i] = c[i] / l;
+        tb = distance_to_boundary(o.geo, t.pos, ch, t.vol, t.surf, &which);
+        // dip rule: on a surface, tangent into the volume but chord out of it -> the helix dips into the volume
+        // for less than this h; halve h (not a substep) instead of crossing with zero travel
+        if (tb == 0.0 && halvings < MAX_DIP_HALVINGS && tangent_points_inward(o.geo, t.pos, t.dir, ch, which)) { h *= 0.5; continue; }
+        break;
+      }
       if (tb <= l) {
         double f = tb / l;
         double pf[3], df[3];

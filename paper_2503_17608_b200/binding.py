@@ -20,7 +20,7 @@ EXPORTS = ["cel_create", "cel_set_stream", "cel_workspace_bytes", "cel_set_works
            "cel_transport_device", "cel_tallies", "cel_destroy", "cel_strerror", "cel_last_cuda_error", "cel_set_option",
            "cel_debug_begin", "cel_debug_step", "cel_debug_read_state", "cel_debug_read_indices",
            "cel_debug_n_initializers", "cel_debug_read_initializers", "cel_debug_n_counts", "cel_debug_read_counts",
-           "cel_debug_table", "cel_debug_uniforms"]
+           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times"]
 
 
 class cel_material(C.Structure):
@@ -89,6 +89,10 @@ def load_library():
     L.cel_debug_read_counts.argtypes = [vp, vp]
     L.cel_debug_table.argtypes = [vp, C.c_int, C.c_int, vp]
     L.cel_debug_uniforms.argtypes = [vp, vp, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, vp]
+    L.cel_kernel_count.restype = C.c_int
+    L.cel_kernel_name.restype = C.c_char_p
+    L.cel_kernel_name.argtypes = [C.c_int]
+    L.cel_kernel_times.argtypes = [vp, vp, vp]
     _lib = L
     return L
 
@@ -183,6 +187,14 @@ class Context:
     def tallies(self):
         """MeV, [n_events][n_bins+1]; last column = escaped energy"""
         return self.tallies_fixed().astype(np.float64) * 2.0 ** -36
+
+    def kernel_times(self):
+        """{kernel name: (device ms, launches)} of the last transport run with option profile=1"""
+        L = load_library()
+        n = L.cel_kernel_count()
+        ms = np.zeros(n); cnt = np.zeros(n, np.uint64)
+        self._check(L.cel_kernel_times(self.h, _p(ms), _p(cnt)), "cel_kernel_times")
+        return {L.cel_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}
 
     # ---- debug / parity surface
     def begin(self, primaries, n_events):

@@ -21,6 +21,7 @@ namespace {
 
 constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action counts are logged
 constexpr int kStatusSlots = 2;
+constexpr int kMaxKernelsPerIteration = 16;
 
 struct HostTables {                 // per material, kept for cel_debug_table
   std::vector<double> t[5];         // compton, pe, pair, brems, range
@@ -55,6 +56,13 @@ struct cel_ctx {
   uint64_t launches = 0; int kernels_per_iteration = 0;
   Control last{};                   // final status of the last run
   std::string cuda_error;
+  // per-kernel device timing (option "profile"): events around every launch, direct launches, one sync per batch
+  int profile = 0;
+  std::vector<cudaEvent_t> prof_ev;   // [batch][kMaxKernelsPerIteration + 1]
+  int prof_b = 0;                     // iteration inside the current batch
+  int iter_kernel[kMaxKernelsPerIteration] = {0};
+  double kernel_ms[CEL_KERNEL_COUNT] = {0};
+  uint64_t kernel_launches[CEL_KERNEL_COUNT] = {0};
 };
 
 namespace {
@@ -318,6 +326,7 @@ extern "C" void cel_destroy(cel_ctx* c) {
   if (c->ev_start) cudaEventDestroy(c->ev_start);
   if (c->ev_stop) cudaEventDestroy(c->ev_stop);
   for (int i = 0; i < kStatusSlots; ++i) if (c->ev_batch[i]) cudaEventDestroy(c->ev_batch[i]);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
   delete c;
 }
@@ -342,6 +351,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   if (!c || !name) return CEL_ERR_INVALID_ARG;
   if (!std::strcmp(name, "use_graph")) c->use_graph = v ? 1 : 0;
   else if (!std::strcmp(name, "batch")) { if (v < 1 || v > 4096) return CEL_ERR_INVALID_ARG; c->batch = (int)v; }
+  else if (!std::strcmp(name, "profile")) c->profile = v ? 1 : 0;
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
   return CEL_OK;
@@ -372,6 +382,17 @@ int physics_grid(const cel_ctx* c) {
   return (int)(need < cap ? need : cap);
 }
 
+const char* const kKernelNames[CEL_KERNEL_COUNT] = {
+    "vac_count", "init_fill", "scatter", "annihilation", "photoelectric", "pair", "compton", "bremsstrahlung",
+    "move_photon", "move_charged", "score", "push_count", "push_write"};
+
+// bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
+inline void after_launch(cel_ctx* c, int id, int& n) {
+  c->iter_kernel[n] = id;
+  ++n;
+  if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1) + n], c->stream);
+}
+
 // one step iteration = P1, P2, P3i, P3m, P4, P5 (docs/PHYSICS_SPEC.md S1); returns the number of kernels enqueued
 int enqueue_iteration(cel_ctx* c) {
   const DeviceState& D = c->D;
@@ -379,22 +400,37 @@ int enqueue_iteration(cel_ctx* c) {
   const int tg = (int)D.n_tiles;
   const int pg = physics_grid(c);
   int n = 0;
-  k_vac_count<<<tg, kTileThreads, 0, s>>>(D); ++n;
-  k_init_fill<<<tg, kTileThreads, 0, s>>>(D); ++n;
-  if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); ++n; }
+  if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1)], s);
+  k_vac_count<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_VAC_COUNT, n);
+  k_init_fill<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_INIT_FILL, n);
+  if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_SCATTER, n); }
   // ANNIH runs first: in the masked modes a positron stopped by the brems kernel of this iteration must not be
   // picked up by the annihilation kernel until the next iteration (S1)
-  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); ++n; }
-  k_interact<A_PE><<<pg, kBlock, 0, s>>>(D); ++n;
-  if (c->phys.enable_pair) { k_interact<A_PAIR><<<pg, kBlock, 0, s>>>(D); ++n; }
-  k_interact<A_COMPTON><<<pg, kBlock, 0, s>>>(D); ++n;
-  if (c->phys.enable_brems) { k_interact<A_BREMS><<<pg, kBlock, 0, s>>>(D); ++n; }
-  k_move_photon<<<pg, kBlock, 0, s>>>(D); ++n;
-  k_move_charged<<<pg, kBlock, 0, s>>>(D); ++n;
-  k_score<<<pg, kBlock, 0, s>>>(D); ++n;
-  k_push_count<<<tg, kTileThreads, 0, s>>>(D); ++n;
-  k_push_write<<<tg, kTileThreads, 0, s>>>(D); ++n;
+  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_ANNIH, n); }
+  k_interact<A_PE><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_PE, n);
+  if (c->phys.enable_pair) { k_interact<A_PAIR><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_PAIR, n); }
+  k_interact<A_COMPTON><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_COMPTON, n);
+  if (c->phys.enable_brems) { k_interact<A_BREMS><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_BREMS, n); }
+  k_move_photon<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_MOVE_G, n);
+  k_move_charged<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_MOVE_C, n);
+  k_score<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_SCORE, n);
+  k_push_count<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH_COUNT, n);
+  k_push_write<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH_WRITE, n);
   return n;
+}
+
+// profile mode: add the event-to-event times of the `n_iter` iterations of the batch that just ended
+int collect_profile(cel_ctx* c, int n_iter, int kernels_per_iteration) {
+  const size_t stride = kMaxKernelsPerIteration + 1;
+  CEL_CUDA(c, cudaEventSynchronize(c->prof_ev[(size_t)(n_iter - 1) * stride + kernels_per_iteration]));
+  for (int b = 0; b < n_iter; ++b)
+    for (int i = 0; i < kernels_per_iteration; ++i) {
+      float ms = 0.f;
+      CEL_CUDA(c, cudaEventElapsedTime(&ms, c->prof_ev[b * stride + i], c->prof_ev[b * stride + i + 1]));
+      c->kernel_ms[c->iter_kernel[i]] += ms;
+      c->kernel_launches[c->iter_kernel[i]] += 1;
+    }
+  return CEL_OK;
 }
 
 // reset slots, staging, counters and tallies; allocate the run's scratch with the stream-ordered allocator
@@ -432,7 +468,16 @@ int prepare_run(cel_ctx* c, uint32_t n_events) {
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
   if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
   if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
-  if (c->use_graph) {
+  for (int i = 0; i < CEL_KERNEL_COUNT; ++i) { c->kernel_ms[i] = 0.0; c->kernel_launches[i] = 0; }
+  if (c->profile) {
+    const size_t need = (size_t)c->batch * (kMaxKernelsPerIteration + 1);
+    while (c->prof_ev.size() < need) {
+      cudaEvent_t e = nullptr;
+      CEL_CUDA(c, cudaEventCreate(&e));
+      c->prof_ev.push_back(e);
+    }
+  }
+  if (c->use_graph && !c->profile) {
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     c->kernels_per_iteration = enqueue_iteration(c);
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
@@ -486,11 +531,15 @@ int run_loop(cel_ctx* c) {
   bool have_prev = false;
   int rc = CEL_OK;
   while (true) {
+    int per_iter = c->kernels_per_iteration;
     for (int b = 0; b < c->batch; ++b) {
-      if (c->use_graph) { CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s)); c->launches += c->kernels_per_iteration; }
-      else c->launches += enqueue_iteration(c);
+      c->prof_b = b;
+      if (c->graph_exec) { CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s)); c->launches += c->kernels_per_iteration; }
+      else { per_iter = enqueue_iteration(c); c->launches += per_iter; }
     }
+    c->prof_b = 0;
     enqueued += c->batch;
+    if (c->profile) { int prc = collect_profile(c, c->batch, per_iter); if (prc != CEL_OK) return prc; }
     CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
     CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
     if (have_prev) {
@@ -547,6 +596,15 @@ extern "C" int cel_tallies(cel_ctx* c, cel_tally_view* out) {
   out->kernel_launches = c->launches;
   if (c->last.error != 0) return c->last.error;
   return c->run_error;
+}
+
+extern "C" int cel_kernel_count(void) { return CEL_KERNEL_COUNT; }
+extern "C" const char* cel_kernel_name(int id) { return (id >= 0 && id < CEL_KERNEL_COUNT) ? kKernelNames[id] : ""; }
+extern "C" int cel_kernel_times(cel_ctx* c, double* ms_out, uint64_t* launches_out) {
+  if (!c || !ms_out || !launches_out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  for (int i = 0; i < CEL_KERNEL_COUNT; ++i) { ms_out[i] = c->kernel_ms[i]; launches_out[i] = c->kernel_launches[i]; }
+  return CEL_OK;
 }
 
 // ================================================================ debug / parity surface (synchronous)

@@ -228,6 +228,18 @@ __device__ __forceinline__ double distance_to_boundary(const Params& P, double x
   which = HIT_Z; return s_z;
 }
 
+// S7.3 dip rule: the tangent d points into the current volume across the surface hit by the chord ch
+// (outward normal: the sign of the chord component for planes, the radial direction for cylinders)
+constexpr int kMaxDipHalvings = 30;
+__device__ __forceinline__ bool tangent_points_inward(const Params& P, double x, double y, double dx, double dy, double dz,
+                                                      double chx, double chy, double chz, int which) {
+  if (which == HIT_Z) return dz * chz < 0.0;
+  if (which == HIT_X) return dx * chx < 0.0;
+  if (which == HIT_Y) return dy * chy < 0.0;
+  const double radial = x * dx + y * dy;
+  return which == HIT_OUTER ? radial < 0.0 : radial > 0.0;
+}
+
 // apply the crossing; dz_sign is the z component of the direction of travel; returns true if escaped
 __device__ __forceinline__ bool cross_boundary(const Params& P, double& z, double dz_travel, int& vol, int& surf, int which) {
   if (P.geom_kind == 0) {

@@ -586,15 +586,21 @@ __global__ void __launch_bounds__(kBlock) k_move_charged(DeviceState D) {
         if (!(s_phys > 0.0)) complete = true;
         while (!complete) {
           if (n == P.max_substeps) break;  // paused
-          const double h = fmin(remaining, h_max);
+          double h = fmin(remaining, h_max);
           const HelixFrame F = helix_frame(P, b.dx, b.dy, b.dz);
-          double nx, ny, nz, ndx, ndy, ndz;
-          helix_point(P, F, a.x, a.y, a.z, omega, h, nx, ny, nz, ndx, ndy, ndz);
-          const double cx = nx - a.x, cy = ny - a.y, cz = nz - a.z;
-          const double l = sqrt(cx * cx + cy * cy + cz * cz);
-          const double chx = cx / l, chy = cy / l, chz = cz / l;
+          double nx, ny, nz, ndx, ndy, ndz, l, chx, chy, chz, tb;
           int which;
-          const double tb = distance_to_boundary(P, a.x, a.y, a.z, chx, chy, chz, vol, surf, which);
+          for (int halvings = 0;; ++halvings) {
+            helix_point(P, F, a.x, a.y, a.z, omega, h, nx, ny, nz, ndx, ndy, ndz);
+            const double cx = nx - a.x, cy = ny - a.y, cz = nz - a.z;
+            l = sqrt(cx * cx + cy * cy + cz * cz);
+            chx = cx / l; chy = cy / l; chz = cz / l;
+            tb = distance_to_boundary(P, a.x, a.y, a.z, chx, chy, chz, vol, surf, which);
+            // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
+            if (tb == 0.0 && halvings < kMaxDipHalvings &&
+                tangent_points_inward(P, a.x, a.y, b.dx, b.dy, b.dz, chx, chy, chz, which)) { h *= 0.5; continue; }
+            break;
+          }
           if (tb <= l) {
             const double f = tb / l;
             double fx, fy, fz, fdx, fdy, fdz;

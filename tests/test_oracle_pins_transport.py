@@ -212,3 +212,39 @@ def test_compton_triangle_closes():
         assert np.abs(resid).max() < 1e-12 * E
         checked += 1
     assert checked > 500
+
+
+def test_dip_rule_no_boundary_ping_pong():
+    """S7.3 dip rule (reading A27): an electron on a Pb/LAr plane whose tangent points shallowly into the
+    LAr while the helix curves back towards the Pb must not oscillate between the two volumes with zero-length steps.
+    Case found in config 3 (event 0, seed 3): T = 45.7 keV, d_z = -0.0082, B = 1 T along x. Pinned by what the
+    mathematics fixes: the track stops by energy loss within a few steps (CSDA range of 46 keV is < 0.01 cm), all of
+    its energy is deposited, nothing goes to the escape bin through the looper cap, and every step moves the track."""
+    geo = W.slab_geometry([0.0, 14.4, 14.63], [1, 0], [0, 1], 20.0, (1.0, 0.0, 0.0))
+    p = W.beam(1, 1, W.ELECTRON, 0.04572788, pos=(-1.9362439, 3.2664487, 14.4))
+    d = np.array([-0.65087321, 0.75914261, -0.0081586]); d /= np.linalg.norm(d)
+    p["dir"] = d
+    o = orc.Oracle(geo, [W.LEAD, W.LAR], phys(3, enable_brems=0), 4, 1)
+    o.begin(p, 1)
+    last = None; stuck = 0; n = 0
+    while n < 200:
+        o.step(); n += 1
+        st = o.state()[0]
+        if st["action"] == VACANT:
+            break
+        cur = tuple(st["pos"])
+        stuck = stuck + 1 if cur == last else 0
+        assert stuck <= 1, "more than one consecutive zero-length step"
+        last = cur
+    assert n < 40
+    T = o.tallies()[0]
+    assert T[-1] == 0.0 and abs(T.sum() - 0.04572788) < 1e-9 * 0.04572788
+
+
+def test_no_track_reaches_looper_cap_in_the_calorimeter():
+    """config 3 has no vacuum: with the dip rule no history is ended by the 2000-step looper cap, so the run length is
+    set by the shower (a few hundred iterations), not by a stuck track"""
+    w = W.config3(n_events=6, n_slots=1 << 13)
+    o = make_oracle(w)
+    o.transport(w.primaries, w.n_events)
+    assert o.counters()["iterations"] < 400
