@@ -483,7 +483,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events) {
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
     CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
   }
-  c->launches = 0; c->run_error = 0; c->ran = true;
+  c->launches = 1; c->run_error = 0; c->ran = true;   // k_reset_state
   std::memset(&c->last, 0, sizeof(Control));
   return CEL_OK;
 }
@@ -517,6 +517,7 @@ int load_primaries_host(cel_ctx* c, const cel_primary* p, uint64_t n) {
   CEL_CUDA(c, cudaMallocAsync(&c->d_prim, bytes ? bytes : 64, s));
   if (n) CEL_CUDA(c, cudaMemcpyAsync(c->d_prim, c->h_prim, bytes, cudaMemcpyHostToDevice, s));
   k_load_primaries<<<c->n_sm, 256, 0, s>>>(c->D, (const PrimaryRec*)c->d_prim, n);
+  c->launches += 1;
   CEL_CUDA(c, cudaGetLastError());
   return CEL_OK;
 }
@@ -575,6 +576,7 @@ extern "C" int cel_transport_device(cel_ctx* c, const void* d_primaries, uint64_
   int rc = prepare_run(c, n_events);
   if (rc != CEL_OK) return rc;
   k_load_primaries<<<c->n_sm, 256, 0, c->stream>>>(c->D, (const PrimaryRec*)d_primaries, n);
+  c->launches += 1;
   CEL_CUDA(c, cudaGetLastError());
   return run_loop(c);
 }
