@@ -33,7 +33,6 @@ SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle"}
 ACTIONS = ("PE", "PAIR", "COMPTON", "MOVE_G", "MOVE_C", "BREMS", "ANNIH", "VACANT")
 STATE_BYTES = 64          # one slot's state: RecA + RecB
 INDEX_BYTES = 4
-STAGE_BYTES = 32
 
 
 def make_workload(name, n_events, n_slots, sort_mode, seed_offset=0):
@@ -168,29 +167,23 @@ def run_reference(args):
 # ---------------------------------------------------------------- algorithmic bytes per kernel
 def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     """bytes each kernel MUST move over one whole transport, from the per-iteration action counts the library logs
-    (64 B state, 4 B index, 1 B key, 32 B deposit stage, 64 B per staged secondary).
+    (64 B state, 4 B index, 1 B key, 64 B per staged secondary; tally atomics stay in L2).
     counts: [iterations][8] action counts after P1. Returns {kernel name: bytes}."""
     c = counts.astype(np.float64).sum(0)
     it = float(len(counts))
     idx = INDEX_BYTES if sort_mode != 0 else 0
-    rw = 2 * STATE_BYTES + idx
+    rw = 2 * STATE_BYTES + idx          # gather + write back one slot through the index
     n = float(n_slots)
-    alive = it * n - c[7]
     sec = float(n_secondaries)
     return {
-        "vac_count": it * n * 1,
-        "init_fill": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES,
+        "init_fill": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES,   # key bytes + (read init, write slot)
         "scatter": it * n * (1 + INDEX_BYTES),
         "annihilation": c[6] * (rw + 2 * STATE_BYTES),
         "photoelectric": c[0] * (rw + STATE_BYTES),
         "pair": c[1] * (rw + 2 * STATE_BYTES),
-        "compton": c[2] * (rw + STATE_BYTES),
-        "bremsstrahlung": c[5] * (rw + STATE_BYTES),
-        "move_photon": (c[3] + c[2]) * rw,
-        "move_charged": (c[4] + c[5]) * rw,
-        "score": alive * (idx + STAGE_BYTES),
-        "push_count": it * n * 1,
-        "push_write": it * n * 1 + sec * 2 * STATE_BYTES,
+        "photon": (c[3] + c[2]) * rw + c[2] * STATE_BYTES,                   # Compton stages one electron
+        "charged": (c[4] + c[5]) * rw + c[5] * STATE_BYTES,                  # bremsstrahlung stages one photon
+        "push": sec * (1 + 2 * STATE_BYTES),                                 # nsec byte + (read staging, write stack)
     }
 
 

@@ -118,10 +118,11 @@ void cel_destroy(cel_ctx*);
 const char* cel_strerror(int code);
 const char* cel_last_cuda_error(cel_ctx*);
 
-/* The kernels of one step iteration, in launch order (S1). P1: VAC_COUNT, INIT_FILL; P2: SCATTER (sorted modes);
- * P3i: ANNIH, PE, PAIR, COMPTON, BREMS; P3m: MOVE_G, MOVE_C; P4: SCORE; P5: PUSH_COUNT, PUSH_WRITE. */
-enum { CEL_K_VAC_COUNT = 0, CEL_K_INIT_FILL, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_COMPTON,
-       CEL_K_BREMS, CEL_K_MOVE_G, CEL_K_MOVE_C, CEL_K_SCORE, CEL_K_PUSH_COUNT, CEL_K_PUSH_WRITE, CEL_KERNEL_COUNT };
+/* The kernels of one step iteration (S1). P1 (+ the P2 histogram): INIT_FILL; P2: SCATTER (sorted modes);
+ * P3i: ANNIH, PE, PAIR; P3i+P3m: PHOTON (Compton, then the photon move), CHARGED (bremsstrahlung, then the charged move
+ * with energy loss and MSC); P4 (scoring) happens inside the action kernels; P5: PUSH. */
+enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
+       CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
 /* Per-kernel device time of the last transport run with option "profile" = 1 (per-kernel HBM
@@ -132,8 +133,10 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
 
 /* Run-time knobs (before a transport). use_graph: replay one captured CUDA graph per iteration (default 1).
  * batch: iterations enqueued between status polls (default 16). max_iterations: safety stop (default 2^22).
- * profile: 1 = launch the kernels directly with a CUDA event after each one and synchronise once per batch, so that
- * cel_kernel_times can report per-kernel device time (a measurement mode: results are identical, the run is slower). */
+ * profile: 1 = launch the kernels directly, one after the other, with a CUDA event after each one and synchronise once
+ * per batch, so that cel_kernel_times can report per-kernel device time (a measurement mode: results are identical,
+ * the run is slower). concurrent: 1 (default) = the independent action kernels of an iteration run as parallel
+ * branches of the iteration graph; 0 = one after the other. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* ---- debug / parity surface (synchronous, not timed) ---- */

@@ -3,6 +3,7 @@
 // No torch types, no CPU fallback: every step of the path runs in the kernels of cel_kernels.cuh.
 #include "../../include/cel.h"
 #include "cel_kernels.cuh"
+#include "cel_physics.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -14,7 +15,7 @@ using namespace cel;
 
 static_assert(sizeof(cel_primary) == 64 && sizeof(PrimaryRec) == 64, "cel_primary layout");
 static_assert(sizeof(cel_track) == 80 && sizeof(TrackRec) == 80, "cel_track layout");
-static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32 && sizeof(Stage) == 32, "record layout");
+static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32, "record layout");
 static_assert(sizeof(DeviceState) < 3500, "DeviceState must fit in kernel parameter space");
 
 namespace {
@@ -22,6 +23,7 @@ namespace {
 constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action counts are logged
 constexpr int kStatusSlots = 2;
 constexpr int kMaxKernelsPerIteration = 16;
+constexpr int kSideStreams = 2;
 
 struct HostTables {                 // per material, kept for cel_debug_table
   std::vector<double> t[5];         // compton, pe, pair, brems, range
@@ -45,6 +47,9 @@ struct cel_ctx {
   // stream-ordered scratch of the current run
   void* scratch = nullptr; void* d_tally = nullptr; void* d_prim = nullptr;
   cudaStream_t stream = nullptr; bool own_stream = false;
+  cudaStream_t side[kSideStreams] = {nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
+  cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr};
+  int concurrent = 1;
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
   Control* h_status = nullptr;      // pinned, kStatusSlots entries
   uint64_t* h_tally = nullptr; size_t h_tally_bytes = 0;   // pinned
@@ -160,20 +165,33 @@ int host_locate(const cel_geometry& g, const double* bounds, const double pos[3]
 namespace {
 
 struct Layout {
-  uint64_t stA, stB, akey, nsec, indices, stage, secA, secB, initA, initB, ctl, log, total;
+  uint64_t stA, stB, akey, nsec, indices, secA, secB, initA, initB, ctl, log, total;
 };
+
+// bookkeeping tiles (cel_device.cuh): sub-tiles of kSub slots, at most kMaxTiles tiles of 2^shift slots
+struct Tiling { uint32_t n_tiles, tile_shift, subs_per_tile; };
+Tiling make_tiling(uint64_t N) {
+  const uint64_t subs = (N + kSub - 1) / kSub;
+  uint32_t spt = 1, shift = 10;
+  static_assert(kSub == 1024, "tile_shift assumes 1024-slot sub-tiles");
+  while ((subs + spt - 1) / spt > (uint64_t)kMaxTiles) { spt *= 2; shift += 1; }
+  Tiling t;
+  t.subs_per_tile = spt; t.tile_shift = shift;
+  t.n_tiles = (uint32_t)((N + ((uint64_t)1 << shift) - 1) >> shift);
+  return t;
+}
 
 Layout make_layout(uint64_t N, uint64_t cap, int sort_mode) {
   Layout L{};
-  const uint64_t tiles = (N + kTile - 1) / kTile;
+  const Tiling tl = make_tiling(N);
+  const uint64_t padded = (uint64_t)tl.n_tiles << tl.tile_shift;
   uint64_t o = 0;
   auto take = [&](uint64_t bytes) { uint64_t r = o; o = align_up(o + bytes, 256); return r; };
   L.stA = take(N * sizeof(RecA));
   L.stB = take(N * sizeof(RecB));
-  L.akey = take(tiles * kTile);
-  L.nsec = take(tiles * kTile);
+  L.akey = take(padded);
+  L.nsec = take(padded);
   L.indices = take(sort_mode != CEL_SORT_NONE ? N * sizeof(uint32_t) : 0);
-  L.stage = take(N * sizeof(Stage));
   L.secA = take(2 * N * sizeof(RecA));
   L.secB = take(2 * N * sizeof(RecB));
   L.initA = take(cap * sizeof(RecA));
@@ -204,7 +222,6 @@ int lay_out(cel_ctx* c) {
   D.stA = (RecA*)(base + L.stA); D.stB = (RecB*)(base + L.stB);
   D.akey = (uint8_t*)(base + L.akey); D.nsec = (uint8_t*)(base + L.nsec);
   D.indices = (D.sort_mode != CEL_SORT_NONE) ? (uint32_t*)(base + L.indices) : nullptr;
-  D.stage = (Stage*)(base + L.stage);
   D.secA = (RecA*)(base + L.secA); D.secB = (RecB*)(base + L.secB);
   D.initA = (RecA*)(base + L.initA); D.initB = (RecB*)(base + L.initB);
   D.ctl = (Control*)(base + L.ctl);
@@ -296,12 +313,18 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   P.u0 = std::log(1e-3); P.du = std::log(10.0) / 64.0; P.inv_du = 1.0 / P.du;
   P.mats = (const MaterialDev*)(db + o_mats); P.photon_xs = (const PhotonXs*)(db + o_ph);
   P.charged_xs = (const ChargedXs*)(db + o_ch); P.range_tab = (const double*)(db + o_rg);
-  D.N = (uint32_t)n_slots; D.n_tiles = (uint32_t)((n_slots + kTile - 1) / kTile);
+  const Tiling tl = make_tiling(n_slots);
+  D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
   D.sort_mode = sort_mode;
   D.init_capacity = default_capacity(n_slots, ph->init_capacity);
 
   if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);
   c->own_stream = true;
+  for (int i = 0; i < kSideStreams; ++i) {
+    if (cudaStreamCreateWithFlags(&c->side[i], cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);
+    if (cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  }
+  if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
   if (cudaEventCreate(&c->ev_start) != cudaSuccess || cudaEventCreate(&c->ev_stop) != cudaSuccess) return fail(CEL_ERR_CUDA);
   for (int i = 0; i < kStatusSlots; ++i)
     if (cudaEventCreateWithFlags(&c->ev_batch[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
@@ -313,6 +336,11 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
 extern "C" void cel_destroy(cel_ctx* c) {
   if (!c) return;
   if (c->stream) cudaStreamSynchronize(c->stream);
+  for (int i = 0; i < kSideStreams; ++i) {
+    if (c->side[i]) { cudaStreamSynchronize(c->side[i]); cudaStreamDestroy(c->side[i]); }
+    if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
+  }
+  if (c->ev_fork) cudaEventDestroy(c->ev_fork);
   if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
   if (c->graph) cudaGraphDestroy(c->graph);
   if (c->scratch) cudaFree(c->scratch);
@@ -352,6 +380,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   if (!std::strcmp(name, "use_graph")) c->use_graph = v ? 1 : 0;
   else if (!std::strcmp(name, "batch")) { if (v < 1 || v > 4096) return CEL_ERR_INVALID_ARG; c->batch = (int)v; }
   else if (!std::strcmp(name, "profile")) c->profile = v ? 1 : 0;
+  else if (!std::strcmp(name, "concurrent")) c->concurrent = v ? 1 : 0;
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
   return CEL_OK;
@@ -383,8 +412,7 @@ int physics_grid(const cel_ctx* c) {
 }
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
-    "vac_count", "init_fill", "scatter", "annihilation", "photoelectric", "pair", "compton", "bremsstrahlung",
-    "move_photon", "move_charged", "score", "push_count", "push_write"};
+    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
@@ -393,29 +421,44 @@ inline void after_launch(cel_ctx* c, int id, int& n) {
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1) + n], c->stream);
 }
 
-// one step iteration = P1, P2, P3i, P3m, P4, P5 (docs/PHYSICS_SPEC.md S1); returns the number of kernels enqueued
+// one step iteration = P1, P2, P3 (+P4 inside the action kernels), P5 (docs/PHYSICS_SPEC.md S1); returns the number of
+// kernels enqueued. The five action kernels touch disjoint slots. Sorted by action, their ranges are fixed by the sort,
+// so they are independent and run as parallel branches (side streams; parallel graph branches under capture). In the
+// masked modes a kernel picks its participants by the key byte, which other kernels rewrite, so the order
+// interaction -> move must hold per species: {ANNIH -> CHARGED} runs beside {PE -> PAIR -> PHOTON}.
 int enqueue_iteration(cel_ctx* c) {
   const DeviceState& D = c->D;
   cudaStream_t s = c->stream;
   const int tg = (int)D.n_tiles;
   const int pg = physics_grid(c);
+  const bool fork = c->concurrent && !c->profile;
   int n = 0;
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1)], s);
-  k_vac_count<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_VAC_COUNT, n);
   k_init_fill<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_INIT_FILL, n);
   if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_SCATTER, n); }
-  // ANNIH runs first: in the masked modes a positron stopped by the brems kernel of this iteration must not be
-  // picked up by the annihilation kernel until the next iteration (S1)
-  if (c->phys.enable_annihilation) { k_interact<A_ANNIH><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_ANNIH, n); }
-  k_interact<A_PE><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_PE, n);
-  if (c->phys.enable_pair) { k_interact<A_PAIR><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_PAIR, n); }
-  k_interact<A_COMPTON><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_COMPTON, n);
-  if (c->phys.enable_brems) { k_interact<A_BREMS><<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_BREMS, n); }
-  k_move_photon<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_MOVE_G, n);
-  k_move_charged<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_MOVE_C, n);
-  k_score<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_SCORE, n);
-  k_push_count<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH_COUNT, n);
-  k_push_write<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH_WRITE, n);
+  cudaStream_t s_photon = s, s_small = s;
+  if (fork) {
+    cudaEventRecord(c->ev_fork, s);
+    cudaStreamWaitEvent(c->side[0], c->ev_fork, 0);
+    s_photon = c->side[0]; s_small = c->side[0];
+    if (D.sort_mode == CEL_SORT_BY_ACTION) { cudaStreamWaitEvent(c->side[1], c->ev_fork, 0); s_small = c->side[1]; }
+  }
+  // chain on the main stream: annihilation (must precede the charged kernel in the masked modes), charged
+  cudaStream_t s_annih = (fork && D.sort_mode == CEL_SORT_BY_ACTION) ? s_small : s;
+  if (c->phys.enable_annihilation) { k_annihilation<<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
+  k_photoelectric<<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PE, n);
+  if (c->phys.enable_pair) { k_pair<<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PAIR, n); }
+  k_photon<<<pg, kBlock, 0, s_photon>>>(D); after_launch(c, CEL_K_PHOTON, n);
+  k_charged<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_CHARGED, n);
+  if (fork) {
+    cudaEventRecord(c->ev_join[0], c->side[0]);
+    cudaStreamWaitEvent(s, c->ev_join[0], 0);
+    if (D.sort_mode == CEL_SORT_BY_ACTION) {
+      cudaEventRecord(c->ev_join[1], c->side[1]);
+      cudaStreamWaitEvent(s, c->ev_join[1], 0);
+    }
+  }
+  k_push<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH, n);
   return n;
 }
 
@@ -443,8 +486,8 @@ int prepare_run(cel_ctx* c, uint32_t n_events) {
   if (c->scratch) { CEL_CUDA(c, cudaFreeAsync(c->scratch, s)); c->scratch = nullptr; }
   if (c->d_tally) { CEL_CUDA(c, cudaFreeAsync(c->d_tally, s)); c->d_tally = nullptr; }
   const uint64_t tiles = D.n_tiles;
-  const uint64_t o_vac = 0, o_hist = align_up(tiles * 4, 256), o_sec = align_up(o_hist + tiles * 32, 256);
-  const uint64_t scratch_bytes = align_up(o_sec + tiles * 4, 256);
+  const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
+  const uint64_t scratch_bytes = align_up(o_hist + tiles * 32, 256);
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
   const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
   CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));

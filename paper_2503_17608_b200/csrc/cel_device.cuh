@@ -29,19 +29,16 @@ enum : uint32_t { PH_INTERACT = 0, PH_STEP = 1, PH_MSC = 2 };
 // of a field-per-array SoA under the index indirection).
 struct __align__(32) RecA { double x, y, z, energy; };
 struct __align__(32) RecB { double dx, dy, dz; unsigned long long meta; };
-// meta: bits 0-3 action | 4-5 ptype | 6 staged | 8-15 vol | 16-23 surf (0xff = none) | 24-39 nsteps | 40-63 event
-struct __align__(32) Stage { long long q_dep, q_esc; uint32_t event; int32_t bin; unsigned long long pad; };
+// meta: bits 0-3 action | 4-5 ptype | 8-15 vol | 16-23 surf (0xff = none) | 24-39 nsteps | 40-63 event
 
 __device__ __forceinline__ int meta_action(unsigned long long m) { return (int)(m & 0xfull); }
 __device__ __forceinline__ int meta_ptype(unsigned long long m) { return (int)((m >> 4) & 0x3ull); }
-__device__ __forceinline__ bool meta_staged(unsigned long long m) { return (m >> 6) & 1ull; }
 __device__ __forceinline__ int meta_vol(unsigned long long m) { return (int)((m >> 8) & 0xffull); }
 __device__ __forceinline__ int meta_surf(unsigned long long m) { int s = (int)((m >> 16) & 0xffull); return s == 0xff ? -1 : s; }
 __device__ __forceinline__ uint32_t meta_nsteps(unsigned long long m) { return (uint32_t)((m >> 24) & 0xffffull); }
 __device__ __forceinline__ uint32_t meta_event(unsigned long long m) { return (uint32_t)(m >> 40); }
-__host__ __device__ __forceinline__ unsigned long long make_meta(int action, int ptype, bool staged, int vol, int surf,
-                                                                 uint32_t nsteps, uint32_t event) {
-  return (unsigned long long)(action & 0xf) | ((unsigned long long)(ptype & 0x3) << 4) | ((unsigned long long)(staged ? 1 : 0) << 6) |
+__host__ __device__ __forceinline__ unsigned long long make_meta(int action, int ptype, int vol, int surf, uint32_t nsteps, uint32_t event) {
+  return (unsigned long long)(action & 0xf) | ((unsigned long long)(ptype & 0x3) << 4) |
          ((unsigned long long)(vol & 0xff) << 8) | ((unsigned long long)((surf < 0 ? 0xff : surf) & 0xff) << 16) |
          ((unsigned long long)(nsteps & 0xffff) << 24) | ((unsigned long long)event << 40);
 }
@@ -67,17 +64,6 @@ __device__ __forceinline__ void store_b(RecB* p, const RecB& r) {
   asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(__double_as_longlong(r.dx)), "l"(__double_as_longlong(r.dy)),
                "l"(__double_as_longlong(r.dz)), "l"(r.meta) : "memory");
 }
-__device__ __forceinline__ Stage load_stage(const Stage* p) {
-  Stage s; unsigned long long w2;
-  asm volatile("ld.global.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(s.q_dep), "=l"(s.q_esc), "=l"(w2), "=l"(s.pad) : "l"(p));
-  s.event = (uint32_t)w2; s.bin = (int32_t)(w2 >> 32);
-  return s;
-}
-__device__ __forceinline__ void store_stage(Stage* p, long long q_dep, long long q_esc, uint32_t event, int32_t bin) {
-  unsigned long long w2 = (unsigned long long)event | ((unsigned long long)(uint32_t)bin << 32);
-  asm volatile("st.global.v4.b64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(q_dep), "l"(q_esc), "l"(w2), "l"(0ull) : "memory");
-}
-
 // ---------------------------------------------------------------- per-context read-only device data
 struct MaterialDev { double inv_X0; };
 struct PhotonXs { double compton, pe, pair, pad; };   // one grid node, 32 B
@@ -101,6 +87,61 @@ struct Params {
   const PhotonXs* photon_xs;   // [n_mats][kGrid]
   const ChargedXs* charged_xs; // [n_mats][kGrid]
   const double* range_tab;     // [n_mats][kGrid]
+};
+
+// ---------------------------------------------------------------- per-run device state
+// Bookkeeping tiles: a tile is `tile_slots` = 2^tile_shift consecutive slots, processed by one block in sub-tiles of
+// kSub slots; the tile size grows with N so that there are never more than kMaxTiles tiles, and every block can
+// form its own exclusive prefix over the per-tile counters with one block reduction (no look-back, no extra pass).
+constexpr int kTileThreads = 256;
+constexpr int kKeysPerThread = 4;
+constexpr int kSub = kTileThreads * kKeysPerThread;  // 1024 slots per sub-tile
+constexpr int kMaxTiles = 2048;
+
+// index ranges of the action kernels in the sorted index array (S2)
+enum KernelRange : int { R_PE = 0, R_PAIR, R_ANNIH, R_PHOTON, R_CHARGED, R_COUNT };
+
+struct Control {
+  unsigned long long n_init;        // I, the initializer stack height
+  unsigned long long track_steps, iterations, secondaries;
+  unsigned long long push_total;    // S of this iteration
+  uint32_t iter;                    // k
+  uint32_t alive;                   // A_k (after P1)
+  uint32_t finished;                // A_k == 0 and I == 0
+  int32_t error;
+  uint32_t offsets[9];              // offsets of the sorted index array, per sort key
+  uint32_t counts[8];               // action counts of this iteration (after P1)
+  uint32_t counts_acc[8];           // accumulators (zero between iterations)
+  uint32_t rb[8], re[8];            // index range of each action kernel for this iteration (KernelRange)
+  uint32_t ticket_fill, ticket_push;
+  uint32_t n_logged;
+  uint32_t vac_total;               // V before the fill of this iteration
+};
+
+// everything a kernel needs; passed by value (fits in the 4 KB parameter space)
+struct DeviceState {
+  Params P;
+  uint32_t N;             // n_slots
+  uint32_t n_tiles;
+  uint32_t tile_shift;    // log2(tile_slots)
+  uint32_t subs_per_tile; // tile_slots / kSub
+  int sort_mode;
+  unsigned long long init_capacity;
+  uint32_t n_events;
+  uint32_t log_capacity;
+  RecA* stA; RecB* stB;
+  uint8_t* akey;          // [n_tiles * tile_slots] action | ptype << 4; padding bytes are 0xff
+  uint8_t* nsec;          // [n_tiles * tile_slots] secondaries staged by the slot in this iteration (0..2)
+  uint32_t* indices;      // [N] (sorted modes)
+  RecA* secA; RecB* secB; // [2N] staged secondaries
+  RecA* initA; RecB* initB; // [init_capacity]
+  unsigned long long* tally; // [n_events][n_bins+1]
+  uint32_t* counts_log;   // [log_capacity][8]
+  Control* ctl;
+  // stream-ordered scratch (cudaMallocAsync, per transport call)
+  uint32_t* tile_vac;     // [n_tiles] vacant slots per tile: += by the action kernels, -= by the fill
+  uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
+  uint32_t* tile_hist;    // [n_tiles][8] per-tile sort-key histogram -> exclusive base per key after k_init_fill
 };
 
 // ---------------------------------------------------------------- S3 Philox4x32-10

@@ -1,0 +1,439 @@
+// cel_physics.cuh — the action kernels of one step iteration (docs/PHYSICS_SPEC.md S1, P3i + P3m + P4):
+//   k_photoelectric  [PE range]            S8 photoelectric
+//   k_pair           [PAIR range]          S8 Bethe-Heitler pair
+//   k_annihilation   [ANNIH range]         S8 annihilation at rest
+//   k_photon         [COMPTON+MOVE_G]      S8 Compton, then S5 photon move (a Compton survivor moves in the same iteration)
+//   k_charged        [MOVE_C+BREMS]        S8 bremsstrahlung, then S7 charged move (step limit, helix, CSDA loss, MSC)
+// Each kernel runs only over its action's contiguous range of the sorted index array; in the masked
+// modes (`none`, `by particle`) it runs over the whole / the particle's range and the dense key byte masks
+// non-participants before any state is read. Scoring (P4, S10) happens here, at the point where the
+// deposit is known: warp-aggregated u64 fixed-point atomics, so no deposit is ever staged in HBM.
+// One thread per sorted index tid; slot = state_indices[tid], identity in mode `none`.
+#pragma once
+#include "cel_device.cuh"
+
+namespace cel {
+
+constexpr int kBlock = 256;  // threads per block of the action kernels
+
+// ---------------------------------------------------------------- warp-aggregated integer adds (S10)
+// Lanes of the currently converged set that hit the same cell are combined first (__match_any_sync), one leader
+// issues the atomic. Integer addition is associative, so the result does not depend on the grouping, on thread
+// order or on the sort mode (BASELINE.json config 3: tallies bit-identical across sort modes).
+__device__ __forceinline__ void warp_aggregated_add64(unsigned long long* base, unsigned long long cell, unsigned long long value) {
+  const unsigned active = __activemask();
+  const unsigned peers = __match_any_sync(active, cell);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  unsigned long long sum = 0;
+  unsigned rem = peers;
+  while (rem) {  // every lane of a peer group walks the same mask
+    const int src = __ffs(rem) - 1;
+    sum += __shfl_sync(peers, value, src);
+    rem &= rem - 1;
+  }
+  if (lane == leader) atomicAdd(base + cell, sum);
+}
+__device__ __forceinline__ void warp_aggregated_add32(uint32_t* base, uint32_t cell, uint32_t value) {
+  const unsigned active = __activemask();
+  const unsigned peers = __match_any_sync(active, cell);
+  if (peers == active) {  // the common case in the sorted modes: the whole warp sits in one tile
+    const uint32_t sum = __reduce_add_sync(active, value);
+    if ((threadIdx.x & 31) == __ffs(active) - 1) atomicAdd(base + cell, sum);
+  } else {
+    atomicAdd(base + cell, value);
+  }
+}
+
+// P4 (S10): q = llrint(e * 2^36) added to tally[event][bin]; bin = bin of the volume at the start of the iteration
+__device__ __forceinline__ void score(const DeviceState& D, uint32_t event, int vol0, double edep, double eesc) {
+  const unsigned long long row = (unsigned long long)event * (unsigned long long)(D.P.n_bins + 1);
+  const long long q_dep = quantise(edep);
+  if (q_dep != 0) {
+    const int bin = __ldg(D.P.vol_bin + vol0);
+    if (bin >= 0) warp_aggregated_add64(D.tally, row + (unsigned long long)bin, (unsigned long long)q_dep);
+  }
+  const long long q_esc = quantise(eesc);
+  if (q_esc != 0) warp_aggregated_add64(D.tally, row + (unsigned long long)D.P.n_bins, (unsigned long long)q_esc);
+}
+
+// ---------------------------------------------------------------- the registers of one track
+struct Track {
+  RecA a;                 // x, y, z, energy
+  double dx, dy, dz;
+  int ptype, vol, surf;
+  uint32_t nsteps, event;
+};
+
+__device__ __forceinline__ void stage_secondary(const DeviceState& D, uint32_t slot, int j, const Track& t, double energy,
+                                                double dx, double dy, double dz, int ptype) {
+  RecA a = t.a; a.energy = energy;
+  RecB b; b.dx = dx; b.dy = dy; b.dz = dz;
+  b.meta = make_meta(ptype == P_GAMMA ? A_MOVE_G : A_MOVE_C, ptype, t.vol, t.surf, 0, t.event);
+  store_a(D.secA + 2ull * slot + j, a);
+  store_b(D.secB + 2ull * slot + j, b);
+}
+
+// a charged track whose kinetic energy dropped below the cut (its energy is already in edep): returns the new action
+__device__ __forceinline__ int stop_charged(const Params& P, int ptype, double& edep) {
+  if (ptype == P_POSITRON) {
+    if (P.enable_annihilation) return A_ANNIH;
+    edep += 2.0 * kElectronMass;
+  }
+  return A_VACANT;
+}
+
+// common epilogue: score, write the slot back, keep the dense key byte and the per-tile counters (vacancies created,
+// secondaries staged) that the scans of the next P5/P1 start from
+__device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, const Track& t, int action, int vol0, double edep,
+                                       double eesc, int nsec, bool write_a) {
+  score(D, t.event, vol0, edep, eesc);
+  RecB b; b.dx = t.dx; b.dy = t.dy; b.dz = t.dz;
+  b.meta = make_meta(action, t.ptype, t.vol, t.surf, t.nsteps, t.event);
+  if (write_a) store_a(D.stA + slot, t.a);
+  store_b(D.stB + slot, b);
+  D.akey[slot] = make_key(action, t.ptype);
+  const uint32_t tile = slot >> D.tile_shift;
+  if (nsec) {
+    D.nsec[slot] = (uint8_t)nsec;
+    warp_aggregated_add32(D.tile_sec, tile, (uint32_t)nsec);
+  }
+  if (action == A_VACANT) warp_aggregated_add32(D.tile_vac, tile, 1u);
+}
+
+__device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
+  Track t;
+  t.a = a; t.dx = b.dx; t.dy = b.dy; t.dz = b.dz;
+  t.ptype = meta_ptype(b.meta); t.vol = meta_vol(b.meta); t.surf = meta_surf(b.meta);
+  t.nsteps = meta_nsteps(b.meta); t.event = meta_event(b.meta);
+  return t;
+}
+
+// ================================================================ P3i: pure interactions (the slot is vacated)
+// Loop over the kernel's index range with a grid-stride loop; `slot` is the gathered slot index.
+#define CEL_FOR_RANGE(RANGE_ID)                                                                             \
+  const Control* ctl = D.ctl;                                                                               \
+  if (ctl->finished) return;                                                                                \
+  const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
+  const uint32_t k_iter = ctl->iter;                                                                        \
+  const Params& P = D.P;                                                                                    \
+  (void)k_iter; (void)P;                                                                                    \
+  for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x)
+
+__device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode != 0) ? D.indices[tid] : tid; }
+
+// S8 photoelectric: the photon's energy goes to an electron along d (or is deposited when electrons are local)
+__global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
+  CEL_FOR_RANGE(R_PE) {
+    const uint32_t slot = slot_of(D, tid);
+    if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PE) continue;
+    const RecB b = load_b(D.stB + slot);
+    if (meta_action(b.meta) != A_PE) continue;
+    Track t = unpack(load_a(D.stA + slot), b);
+    double edep = 0.0;
+    int nsec = 0;
+    if (P.electrons_local) edep += t.a.energy;
+    else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
+    finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+  }
+}
+
+// S8 pair: uniform sharing of E - 2 m_e, both collinear; staging order e-, e+
+__global__ void __launch_bounds__(kBlock) k_pair(DeviceState D) {
+  CEL_FOR_RANGE(R_PAIR) {
+    const uint32_t slot = slot_of(D, tid);
+    if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PAIR) continue;
+    const RecB b = load_b(D.stB + slot);
+    if (meta_action(b.meta) != A_PAIR) continue;
+    Track t = unpack(load_a(D.stA + slot), b);
+    double edep = 0.0;
+    int nsec = 0;
+    double xi0, xi1;
+    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+    const double Tav = t.a.energy - 2.0 * kElectronMass;
+    const double Tm = xi0 * Tav;
+    const double Tp = Tav - Tm;
+    if (Tm >= P.cut) stage_secondary(D, slot, nsec++, t, Tm, t.dx, t.dy, t.dz, P_ELECTRON);
+    else edep += Tm;
+    stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
+    finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+  }
+}
+
+// S8 annihilation at rest: two photons of m_e, back to back, isotropic
+__global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
+  CEL_FOR_RANGE(R_ANNIH) {
+    const uint32_t slot = slot_of(D, tid);
+    if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_ANNIH) continue;
+    const RecB b = load_b(D.stB + slot);
+    if (meta_action(b.meta) != A_ANNIH) continue;
+    Track t = unpack(load_a(D.stA + slot), b);
+    double xi0, xi1;
+    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+    const double cost = 2.0 * xi0 - 1.0;
+    const double sint = sqrt(1.0 - cost * cost);
+    double sp, cp;
+    sincos(2.0 * kPi * xi1, &sp, &cp);
+    const double ux = sint * cp, uy = sint * sp, uz = cost;
+    stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
+    stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
+    finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
+  }
+}
+
+// ================================================================ photons: Compton (S8) then move (S5)
+// S8 Compton: Klein-Nishina epsilon-mixture rejection; returns false if the photon fell below the cut (absorbed)
+__device__ __forceinline__ bool compton(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, int& nsec) {
+  const Params& P = D.P;
+  const double E = t.a.energy;
+  const double k = E / kElectronMass;
+  const double e0 = 1.0 / (1.0 + 2.0 * k);
+  const double a1 = -log(e0);
+  const double a2 = (1.0 - e0 * e0) / 2.0;
+  double eps, tt, sin2, xphi;
+  for (uint32_t trial = 0;; ++trial) {
+    double xa, xb, xc;
+    draw_pair(P, slot, k_iter, PH_INTERACT, 2 * trial, xa, xb);
+    draw_pair(P, slot, k_iter, PH_INTERACT, 2 * trial + 1, xc, xphi);
+    if (xa * (a1 + a2) < a1) eps = exp(-a1 * xb);
+    else eps = sqrt(e0 * e0 + (1.0 - e0 * e0) * xb);
+    tt = (1.0 - eps) / (k * eps);
+    sin2 = tt * (2.0 - tt);
+    if (xc <= 1.0 - eps * sin2 / (1.0 + eps * eps) || trial >= 65535u) break;
+  }
+  const double cost = 1.0 - tt;
+  const double sint = sqrt(sin2 > 0.0 ? sin2 : 0.0);
+  const double E1 = eps * E;
+  double d1x = t.dx, d1y = t.dy, d1z = t.dz;
+  rotate_dir(d1x, d1y, d1z, cost, sint, 2.0 * kPi * xphi);
+  const double Te = E - E1;
+  if (P.electrons_local || Te < P.cut) {
+    edep += Te;
+  } else {
+    double ex = E * t.dx - E1 * d1x, ey = E * t.dy - E1 * d1y, ez = E * t.dz - E1 * d1z;
+    const double n = sqrt(ex * ex + ey * ey + ez * ez);
+    if (n > 0.0) { ex /= n; ey /= n; ez /= n; } else { ex = t.dx; ey = t.dy; ez = t.dz; }
+    stage_secondary(D, slot, nsec++, t, Te, ex, ey, ez, P_ELECTRON);
+  }
+  if (E1 < P.cut) { edep += E1; return false; }
+  t.a.energy = E1; t.dx = d1x; t.dy = d1y; t.dz = d1z;
+  return true;
+}
+
+// S5 photon move: sampled free path vs distance to boundary; returns the next action
+__device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& eesc) {
+  const Params& P = D.P;
+  const int vol0 = t.vol;
+  const int mat = __ldg(P.vol_material + t.vol);
+  double sPE = 0.0, sPair = 0.0, sC = 0.0;
+  if (mat >= 0) {
+    const GridPos g = grid_locate(P, t.a.energy);
+    const double2* xs = reinterpret_cast<const double2*>(P.photon_xs + (size_t)mat * kGrid + g.j);  // nodes j, j+1: 64 B
+    const double2 n0a = __ldg(xs), n0b = __ldg(xs + 1), n1a = __ldg(xs + 2), n1b = __ldg(xs + 3);
+    sC = lerp_node(n0a.x, n1a.x, g.f);
+    sPE = lerp_node(n0a.y, n1a.y, g.f);
+    sPair = lerp_node(n0b.x, n1b.x, g.f);
+  }
+  const double stot = (sPE + sPair) + sC;
+  double xi0, xi1;
+  draw_pair(P, slot, k_iter, PH_STEP, 0, xi0, xi1);
+  const double s_d = (stot > 0.0) ? -log(xi0) / stot : CEL_INF;
+  const double x = xi1 * stot;
+  const int process = (x < sPE) ? A_PE : ((x < sPE + sPair) ? A_PAIR : A_COMPTON);
+  int which;
+  const double s_b = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, which);
+  if (t.nsteps < 65535u) t.nsteps += 1;
+  if (s_d < s_b) {
+    t.a.x += s_d * t.dx; t.a.y += s_d * t.dy; t.a.z += s_d * t.dz;
+    t.surf = -1;
+    return process;
+  }
+  t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
+  const bool escaped = cross_boundary(P, t.a.z, t.dz, t.vol, t.surf, which);
+  if (escaped) {
+    eesc += t.a.energy;
+    if (t.vol < 0 || t.vol > 254) t.vol = vol0;
+    return A_VACANT;
+  }
+  return A_MOVE_G;
+}
+
+__global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
+  CEL_FOR_RANGE(R_PHOTON) {
+    const uint32_t slot = slot_of(D, tid);
+    if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_COMPTON && ak != A_MOVE_G) continue; }
+    const RecB b = load_b(D.stB + slot);
+    const int act = meta_action(b.meta);
+    if (act != A_COMPTON && act != A_MOVE_G) continue;
+    Track t = unpack(load_a(D.stA + slot), b);
+    const int vol0 = t.vol;
+    double edep = 0.0, eesc = 0.0;
+    int nsec = 0;
+    int action = A_VACANT;
+    bool alive = true;
+    if (act == A_COMPTON) alive = compton(D, slot, k_iter, t, edep, nsec);
+    if (alive) action = move_photon(D, slot, k_iter, t, eesc);
+    finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+  }
+}
+
+// ================================================================ charged: bremsstrahlung (S8) then move (S7)
+// S7: step limit -> linear or helical propagation (<= max_substeps chord substeps) -> CSDA loss -> MSC -> fate
+__device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, double& eesc) {
+  const Params& P = D.P;
+  const int vol0 = t.vol;
+  const int ptype = t.ptype;
+  if (t.nsteps < 65535u) t.nsteps += 1;
+  const double T0 = t.a.energy;
+  if (T0 < P.cut) {  // S7.1
+    edep += T0;
+    t.a.energy = 0.0;
+    return stop_charged(P, ptype, edep);
+  }
+  const int mat = __ldg(P.vol_material + t.vol);
+  const double p = sqrt(T0 * (T0 + 2.0 * kElectronMass));
+  const double beta = p / (T0 + kElectronMass);
+  // S7.2 step limit
+  double r0 = 0.0, s_r = CEL_INF, s_d = CEL_INF;
+  int j0 = 0;
+  if (mat >= 0) {
+    const GridPos g = grid_locate(P, T0);
+    j0 = g.j;
+    const double2* cxs = reinterpret_cast<const double2*>(P.charged_xs + (size_t)mat * kGrid + g.j);  // nodes j, j+1
+    const double2 n0 = __ldg(cxs);
+    const double2 n1 = __ldg(cxs + 1);
+    if (P.enable_eloss) {
+      r0 = lerp_node(n0.y, n1.y, g.f);
+      s_r = (r0 <= kRhoF) ? r0 : fmax(kAlphaR * r0, kRhoF);
+    }
+    const double sb = lerp_node(n0.x, n1.x, g.f);
+    double xi0, xi1;
+    draw_pair(P, slot, k_iter, PH_STEP, 0, xi0, xi1);
+    if (sb > 0.0) s_d = -log(xi0) / sb;
+  }
+  const bool interaction_wins = s_d < s_r;
+  const double s_phys = interaction_wins ? s_d : s_r;
+  // S7.3 propagation
+  double travelled = 0.0;
+  bool escaped = false, complete = false;
+  if (P.bmag == 0.0) {
+    int which;
+    const double s_b = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, which);
+    if (s_phys < s_b) {
+      t.a.x += s_phys * t.dx; t.a.y += s_phys * t.dy; t.a.z += s_phys * t.dz;
+      t.surf = -1; travelled = s_phys; complete = true;
+    } else {
+      t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
+      travelled = s_b;
+      escaped = cross_boundary(P, t.a.z, t.dz, t.vol, t.surf, which);
+    }
+  } else {
+    const double q = (ptype == P_ELECTRON) ? -1.0 : 1.0;
+    const double omega = q * kKappa * P.bmag / p;
+    const double h_max = fmin(sqrt(8.0 * kDeltaChord / fabs(omega)), 0.5 / fabs(omega));
+    double remaining = s_phys;
+    int n = 0;
+    if (!(s_phys > 0.0)) complete = true;
+    while (!complete) {
+      if (n == P.max_substeps) break;  // paused: the remainder is re-sampled next iteration
+      double h = fmin(remaining, h_max);
+      const HelixFrame F = helix_frame(P, t.dx, t.dy, t.dz);
+      double nx, ny, nz, ndx, ndy, ndz, l, chx, chy, chz, tb;
+      int which;
+      for (int halvings = 0;; ++halvings) {
+        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, h, nx, ny, nz, ndx, ndy, ndz);
+        const double cx = nx - t.a.x, cy = ny - t.a.y, cz = nz - t.a.z;
+        l = sqrt(cx * cx + cy * cy + cz * cz);
+        chx = cx / l; chy = cy / l; chz = cz / l;
+        tb = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, chx, chy, chz, t.vol, t.surf, which);
+        // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
+        if (tb == 0.0 && halvings < kMaxDipHalvings &&
+            tangent_points_inward(P, t.a.x, t.a.y, t.dx, t.dy, t.dz, chx, chy, chz, which)) { h *= 0.5; continue; }
+        break;
+      }
+      if (tb <= l) {
+        const double f = tb / l;
+        double fx, fy, fz, fdx, fdy, fdz;
+        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, f * h, fx, fy, fz, fdx, fdy, fdz);
+        t.a.x += tb * chx; t.a.y += tb * chy; t.a.z += tb * chz;
+        normalise3(fdx, fdy, fdz);
+        t.dx = fdx; t.dy = fdy; t.dz = fdz;
+        travelled += f * h;
+        escaped = cross_boundary(P, t.a.z, chz, t.vol, t.surf, which);
+        break;
+      }
+      normalise3(ndx, ndy, ndz);
+      t.a.x = nx; t.a.y = ny; t.a.z = nz;
+      t.dx = ndx; t.dy = ndy; t.dz = ndz;
+      travelled += h;
+      t.surf = -1;
+      remaining -= h;
+      n += 1;
+      if (remaining <= 0.0) { travelled = s_phys; complete = true; }
+    }
+  }
+  // S7.4 energy loss
+  double T1 = T0;
+  if (mat >= 0 && P.enable_eloss) {
+    const double r1 = r0 - travelled;
+    T1 = (r1 <= 0.0) ? 0.0 : range_inverse(P, P.range_tab + (size_t)mat * kGrid, r1, j0);
+    if (T1 > T0) T1 = T0;
+    edep += T0 - T1;
+  }
+  // S7.5 multiple scattering
+  if (P.enable_msc && !escaped && mat >= 0 && travelled > 0.0 && T1 >= P.cut) {
+    const double x = travelled * __ldg(&P.mats[mat].inv_X0);
+    const double theta0 = 13.6 / (beta * p) * sqrt(x) * fmax(0.0, 1.0 + 0.038 * log(x));
+    double xm0, xm1;
+    draw_pair(P, slot, k_iter, PH_MSC, 0, xm0, xm1);
+    const double theta = fmin(theta0 * sqrt(-2.0 * log(xm0)), kPi);
+    double st, ct;
+    sincos(theta, &st, &ct);
+    rotate_dir(t.dx, t.dy, t.dz, ct, st, 2.0 * kPi * xm1);
+  }
+  // S7.6 fate
+  const double rest = (ptype == P_POSITRON) ? 2.0 * kElectronMass : 0.0;
+  if (escaped) {
+    eesc += T1 + rest; t.a.energy = T1;
+    if (t.vol < 0 || t.vol > 254) t.vol = vol0;
+    return A_VACANT;
+  }
+  if (T1 < P.cut) {
+    edep += T1; t.a.energy = 0.0;
+    return stop_charged(P, ptype, edep);
+  }
+  if (t.nsteps >= P.max_steps_per_track) {
+    eesc += T1 + rest; t.a.energy = T1;
+    return A_VACANT;
+  }
+  t.a.energy = T1;
+  return (interaction_wins && complete) ? A_BREMS : A_MOVE_C;
+}
+
+__global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
+  CEL_FOR_RANGE(R_CHARGED) {
+    const uint32_t slot = slot_of(D, tid);
+    if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }
+    const RecB b = load_b(D.stB + slot);
+    const int act = meta_action(b.meta);
+    if (act != A_MOVE_C && act != A_BREMS) continue;
+    Track t = unpack(load_a(D.stA + slot), b);
+    const int vol0 = t.vol;
+    double edep = 0.0, eesc = 0.0;
+    int nsec = 0;
+    int action = A_MOVE_C;
+    if (act == A_BREMS) {  // S8: k log-uniform on [k_c, T]; photon collinear
+      double xi0, xi1;
+      draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+      const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
+      stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
+      const double T1 = t.a.energy - kph;
+      if (T1 < P.cut) { edep += T1; t.a.energy = 0.0; action = stop_charged(P, t.ptype, edep); }
+      else t.a.energy = T1;
+    }
+    if (action == A_MOVE_C) action = move_charged(D, slot, k_iter, t, edep, eesc);
+    finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+  }
+}
+
+}  // namespace cel
