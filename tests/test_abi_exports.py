@@ -25,7 +25,7 @@ def test_library_exports_every_declared_symbol():
     assert L.cel_strerror(0) == b"ok" and L.cel_strerror(-4) == b"initializer stack overflow"
     # workspace size is pure host arithmetic
     n = binding.workspace_bytes(1 << 20, 1 << 24, 1)
-    assert n > (1 << 20) * (64 + 32 + 128 + 4) + (1 << 24) * 64
+    assert n > (1 << 20) * (64 + 128 + 4 + 2) + (1 << 24) * 64  # state + secondary staging + index + key bytes, stack
 
 
 def test_struct_layouts_match_header():
