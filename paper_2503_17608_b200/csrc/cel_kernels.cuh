@@ -215,26 +215,56 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   }
   if (!last_block_done(&ctl->ticket_fill)) return;
   // ---- last block: vacancies left per tile, per-key exclusive scan over tiles, offsets, ranges, counters
-  {
-    __shared__ uint32_t carry_v;
-    if (threadIdx.x == 0) carry_v = 0;
-    __syncthreads();
-    for (uint32_t b0 = 0; b0 < D.n_tiles; b0 += kTileThreads) {
-      const uint32_t i = b0 + threadIdx.x;
-      const uint32_t v = (i < D.n_tiles) ? D.tile_vac[i] : 0;
-      uint32_t total;
-      const uint32_t ex = carry_v + block_excl_scan(v, smem, total);
-      if (i < D.n_tiles) D.tile_vac[i] = v - min(v, n_take > ex ? n_take - ex : 0u);
-      __syncthreads();
-      if (threadIdx.x == 0) carry_v += total;
-      __syncthreads();
+  {  // tile t keeps v - (filled in t), filled = min(v, max(0, n_take - (vacancies before t))); thread owns `per` tiles
+    const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;
+    const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
+    uint32_t v[kMaxTiles / kTileThreads];
+    uint32_t sum = 0;
+#pragma unroll
+    for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) { v[i] = (t0 + i < t1) ? D.tile_vac[t0 + i] : 0; sum += v[i]; }
+    uint32_t total;
+    uint32_t ex = block_excl_scan(sum, smem, total);
+#pragma unroll
+    for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) {
+      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - min(v[i], n_take > ex ? n_take - ex : 0u);
+      ex += v[i];
     }
   }
+  // per-key exclusive scan of tile_hist over the tiles, all keys in one pass: thread t owns `per` consecutive tiles
   __shared__ uint32_t key_total[8];
+  __shared__ uint32_t warp_tot[kTileThreads / 32][8];
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
-  for (int k = 0; k < n_keys; ++k) {
-    uint32_t t = block_scan_array(D.tile_hist + k, D.n_tiles, 8, smem);
-    if (threadIdx.x == 0) key_total[k] = t;
+  if (n_keys) {
+    const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;   // <= kMaxTiles / 256 = 8
+    const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
+    uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (uint32_t t = t0; t < t1; ++t) {
+      const uint4 a = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8), b = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8 + 4);
+      acc[0] += a.x; acc[1] += a.y; acc[2] += a.z; acc[3] += a.w; acc[4] += b.x; acc[5] += b.y; acc[6] += b.z; acc[7] += b.w;
+    }
+    uint32_t ex[8];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const uint32_t incl = warp_incl_scan(acc[k]);
+      ex[k] = incl - acc[k];
+      if (lane == 31) warp_tot[warp][k] = incl;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      uint32_t before = 0, all = 0;
+#pragma unroll
+      for (int w = 0; w < kTileThreads / 32; ++w) { const uint32_t v = warp_tot[w][k]; all += v; if (w < warp) before += v; }
+      ex[k] += before;
+      if (threadIdx.x == 0) key_total[k] = all;
+    }
+    for (uint32_t t = t0; t < t1; ++t) {
+      uint4* pa = reinterpret_cast<uint4*>(D.tile_hist + t * 8); uint4* pb = reinterpret_cast<uint4*>(D.tile_hist + t * 8 + 4);
+      const uint4 a = *pa, b = *pb;
+      *pa = make_uint4(ex[0], ex[1], ex[2], ex[3]); *pb = make_uint4(ex[4], ex[5], ex[6], ex[7]);
+      ex[0] += a.x; ex[1] += a.y; ex[2] += a.z; ex[3] += a.w; ex[4] += b.x; ex[5] += b.y; ex[6] += b.z; ex[7] += b.w;
+    }
     __syncthreads();
   }
   if (threadIdx.x == 0) {
