@@ -275,7 +275,8 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   const uint64_t o_ph = align_up(o_mats + n_mats * sizeof(MaterialDev), 256);
   const uint64_t o_ch = align_up(o_ph + (uint64_t)n_mats * kGrid * sizeof(PhotonXs), 256);
   const uint64_t o_rg = align_up(o_ch + (uint64_t)n_mats * kGrid * sizeof(ChargedXs), 256);
-  const uint64_t blob_bytes = align_up(o_rg + (uint64_t)n_mats * kGrid * sizeof(double), 256);
+  const uint64_t o_en = align_up(o_rg + (uint64_t)n_mats * kGrid * sizeof(double), 256);
+  const uint64_t blob_bytes = align_up(o_en + (uint64_t)kGrid * sizeof(double), 256);
   std::vector<char> blob(blob_bytes, 0);
   std::memcpy(blob.data() + o_bounds, c->h_bounds.data(), (g->n_vol + 1) * sizeof(double));
   std::memcpy(blob.data() + o_vm, c->h_vol_material.data(), g->n_vol * sizeof(int));
@@ -290,6 +291,7 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
       ((double*)(blob.data() + o_rg))[(size_t)m * kGrid + j] = c->tables[m].t[4][j];
     }
   }
+  for (int j = 0; j < kGrid; ++j) ((double*)(blob.data() + o_en))[j] = std::exp(std::log(1e-3) + j * (std::log(10.0) / 64.0));
   auto fail = [&](int code) { cel_destroy(c); return code; };
   if (cudaMalloc(&c->d_params_blob, blob_bytes) != cudaSuccess) return fail(CEL_ERR_OOM);
   if (cudaMemcpy(c->d_params_blob, blob.data(), blob_bytes, cudaMemcpyHostToDevice) != cudaSuccess) return fail(CEL_ERR_CUDA);
@@ -313,6 +315,7 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   P.u0 = std::log(1e-3); P.du = std::log(10.0) / 64.0; P.inv_du = 1.0 / P.du;
   P.mats = (const MaterialDev*)(db + o_mats); P.photon_xs = (const PhotonXs*)(db + o_ph);
   P.charged_xs = (const ChargedXs*)(db + o_ch); P.range_tab = (const double*)(db + o_rg);
+  P.energy_nodes = (const double*)(db + o_en);
   const Tiling tl = make_tiling(n_slots);
   D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
   D.sort_mode = sort_mode;
@@ -448,8 +451,12 @@ int enqueue_iteration(cel_ctx* c) {
   if (c->phys.enable_annihilation) { k_annihilation<<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
   k_photoelectric<<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PE, n);
   if (c->phys.enable_pair) { k_pair<<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PAIR, n); }
-  k_photon<<<pg, kBlock, 0, s_photon>>>(D); after_launch(c, CEL_K_PHOTON, n);
-  k_charged<<<pg, kBlock, 0, s>>>(D); after_launch(c, CEL_K_CHARGED, n);
+  const bool cyl = D.P.geom_kind == CEL_GEOM_CYL, field = D.P.bmag != 0.0;
+  if (cyl) k_photon<1><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0><<<pg, kBlock, 0, s_photon>>>(D);
+  after_launch(c, CEL_K_PHOTON, n);
+  if (cyl) { if (field) k_charged<true, 1><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 1><<<pg, kBlock, 0, s>>>(D); }
+  else { if (field) k_charged<true, 0><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0><<<pg, kBlock, 0, s>>>(D); }
+  after_launch(c, CEL_K_CHARGED, n);
   if (fork) {
     cudaEventRecord(c->ev_join[0], c->side[0]);
     cudaStreamWaitEvent(s, c->ev_join[0], 0);

@@ -87,6 +87,7 @@ struct Params {
   const PhotonXs* photon_xs;   // [n_mats][kGrid]
   const ChargedXs* charged_xs; // [n_mats][kGrid]
   const double* range_tab;     // [n_mats][kGrid]
+  const double* energy_nodes;  // [kGrid] E_j = exp(u_j)
 };
 
 // ---------------------------------------------------------------- per-run device state
@@ -160,8 +161,10 @@ __device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint3
   return o;
 }
 __device__ __forceinline__ double to_uniform(uint32_t lo, uint32_t hi) {
-  unsigned long long x = ((unsigned long long)hi << 32) | lo;
-  return ((double)(x >> 12) + 0.5) * (1.0 / 4503599627370496.0);
+  // ((x >> 12) + 0.5) * 2^-52, exactly: the 52 bits become the mantissa of a double in [1, 2); subtracting 1 and adding
+  // 2^-53 are both exact (the sum has at most 53 significant bits below 1)
+  const unsigned long long x = ((unsigned long long)hi << 32) | lo;
+  return (__longlong_as_double((long long)(0x3ff0000000000000ull | (x >> 12))) - 1.0) + 1.1102230246251565e-16;
 }
 // the two draws (2b, 2b+1) of block b of a phase
 __device__ __forceinline__ void draw_pair(const Params& P, uint32_t slot, uint32_t k, uint32_t phase, uint32_t block, double& xa, double& xb) {
@@ -173,7 +176,7 @@ __device__ __forceinline__ void draw_pair(const Params& P, uint32_t slot, uint32
 // ---------------------------------------------------------------- S4 table lookups
 struct GridPos { int j; double f; };
 __device__ __forceinline__ GridPos grid_locate(const Params& P, double E) {
-  double t = (log(E) - P.u0) / P.du;
+  double t = (log(E) - P.u0) * P.inv_du;
   double fl = floor(t);
   int j = fl < 0.0 ? 0 : (fl > 575.0 ? 575 : (int)fl);
   GridPos g; g.j = j; g.f = t - (double)j;
@@ -185,29 +188,36 @@ __device__ __forceinline__ double lerp_node(double y0, double y1, double f) { re
 __device__ __forceinline__ double range_inverse(const Params& P, const double* __restrict__ R, double r, int j_hint) {
   int j = j_hint;
   while (j > 0 && __ldg(R + j) > r) --j;
-  double Rj = __ldg(R + j), Rj1 = __ldg(R + j + 1);
-  double u = P.u0 + j * P.du + P.du * (r - Rj) / (Rj1 - Rj);
-  return exp(u);
+  const double Rj = __ldg(R + j), Rj1 = __ldg(R + j + 1);
+  // T = exp(u_j + x) = E_j * exp(x), x = du (r - R_j)/(R_j+1 - R_j) in [0, du], du = ln(10)/64 = 0.036:
+  // the degree-8 Taylor polynomial of exp is exact to 1e-17 there
+  const double x = P.du * (r - Rj) / (Rj1 - Rj);
+  double e = 1.0 / 40320.0;
+  e = e * x + 1.0 / 5040.0; e = e * x + 1.0 / 720.0; e = e * x + 1.0 / 120.0; e = e * x + 1.0 / 24.0;
+  e = e * x + 1.0 / 6.0; e = e * x + 0.5; e = e * x + 1.0; e = e * x + 1.0;
+  return __ldg(P.energy_nodes + j) * e;
 }
 
 // ---------------------------------------------------------------- vectors
 __device__ __forceinline__ void normalise3(double& x, double& y, double& z) {
-  double n = sqrt(x * x + y * y + z * z);
-  x /= n; y /= n; z /= n;
+  const double inv = 1.0 / sqrt(x * x + y * y + z * z);
+  x *= inv; y *= inv; z *= inv;
 }
 
 // S8 rotate(d, theta, phi) taking cos(theta), sin(theta)
-__device__ __forceinline__ void rotate_dir(double& dx, double& dy, double& dz, double ct, double st, double phi) {
+// phi = 2 pi xi is passed as xi2 = 2 xi (sincospi: no argument reduction against pi needed)
+__device__ __forceinline__ void rotate_dir(double& dx, double& dy, double& dz, double ct, double st, double xi2) {
   double sp, cp;
-  sincos(phi, &sp, &cp);
+  sincospi(xi2, &sp, &cp);
   double srho = sqrt(dx * dx + dy * dy);
   double ox, oy, oz;
   if (srho == 0.0) {
     double sg = dz < 0.0 ? -1.0 : 1.0;
     ox = st * cp; oy = st * sp; oz = sg * ct;
   } else {
-    ox = dx * ct + st * (dx * dz * cp - dy * sp) / srho;
-    oy = dy * ct + st * (dy * dz * cp + dx * sp) / srho;
+    const double st_rho = st / srho;
+    ox = dx * ct + st_rho * (dx * dz * cp - dy * sp);
+    oy = dy * ct + st_rho * (dy * dz * cp + dx * sp);
     oz = dz * ct - srho * st * cp;
   }
   normalise3(ox, oy, oz);
@@ -220,16 +230,26 @@ enum : int { HIT_Z = 1, HIT_X = 2, HIT_Y = 3, HIT_INNER = 4, HIT_OUTER = 5 };
 
 __device__ __forceinline__ double clamp0(double s) { return s < 0.0 ? 0.0 : s; }
 
+// Distance along d to the boundary of `vol`, and which surface is hit. Callers only use the result when it is
+// <= s_lim (the boundary wins ties against the physics / chord length), so the slab version divides only for the
+// candidates that can be <= s_lim: a candidate num/den with |num| > s_lim |den| (1 + 1e-9) is certainly larger and is
+// left at +inf. Whenever the true minimum is <= s_lim the value and the tie order z, x, y are exactly those of S6.
+constexpr double kFilterSlack = 1.000000001;
+__device__ __forceinline__ double slab_candidate(double num, double den, double s_lim) {
+  if (fabs(num) > s_lim * fabs(den) * kFilterSlack) return CEL_INF;
+  return clamp0(num / den);
+}
+template <int GEOM>
 __device__ __forceinline__ double distance_to_boundary(const Params& P, double x, double y, double z, double dx, double dy, double dz,
-                                                       int vol, int surf, int& which) {
-  if (P.geom_kind == 0) {
+                                                       int vol, int surf, double s_lim, int& which) {
+  if (GEOM == 0) {
     double sz = CEL_INF, sx = CEL_INF, sy = CEL_INF;
-    if (dz > 0.0) sz = clamp0((__ldg(P.bounds + vol + 1) - z) / dz);
-    else if (dz < 0.0) sz = clamp0((__ldg(P.bounds + vol) - z) / dz);
-    if (dx > 0.0) sx = clamp0((P.half_x - x) / dx);
-    else if (dx < 0.0) sx = clamp0((-P.half_x - x) / dx);
-    if (dy > 0.0) sy = clamp0((P.half_y - y) / dy);
-    else if (dy < 0.0) sy = clamp0((-P.half_y - y) / dy);
+    if (dz > 0.0) sz = slab_candidate(__ldg(P.bounds + vol + 1) - z, dz, s_lim);
+    else if (dz < 0.0) sz = slab_candidate(__ldg(P.bounds + vol) - z, dz, s_lim);
+    if (dx > 0.0) sx = slab_candidate(P.half_x - x, dx, s_lim);
+    else if (dx < 0.0) sx = slab_candidate(-P.half_x - x, dx, s_lim);
+    if (dy > 0.0) sy = slab_candidate(P.half_y - y, dy, s_lim);
+    else if (dy < 0.0) sy = slab_candidate(-P.half_y - y, dy, s_lim);
     if (sz <= sx && sz <= sy) { which = HIT_Z; return sz; }
     if (sx <= sy) { which = HIT_X; return sx; }
     which = HIT_Y; return sy;
@@ -282,8 +302,9 @@ __device__ __forceinline__ bool tangent_points_inward(const Params& P, double x,
 }
 
 // apply the crossing; dz_sign is the z component of the direction of travel; returns true if escaped
+template <int GEOM>
 __device__ __forceinline__ bool cross_boundary(const Params& P, double& z, double dz_travel, int& vol, int& surf, int which) {
-  if (P.geom_kind == 0) {
+  if (GEOM == 0) {
     surf = -1;
     if (which != HIT_Z) return true;
     if (dz_travel > 0.0) { z = __ldg(P.bounds + vol + 1); vol += 1; }

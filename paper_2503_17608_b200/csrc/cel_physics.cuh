@@ -173,7 +173,7 @@ __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
     const double cost = 2.0 * xi0 - 1.0;
     const double sint = sqrt(1.0 - cost * cost);
     double sp, cp;
-    sincos(2.0 * kPi * xi1, &sp, &cp);
+    sincospi(2.0 * xi1, &sp, &cp);
     const double ux = sint * cp, uy = sint * sp, uz = cost;
     stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
     stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
@@ -205,7 +205,7 @@ __device__ __forceinline__ bool compton(const DeviceState& D, uint32_t slot, uin
   const double sint = sqrt(sin2 > 0.0 ? sin2 : 0.0);
   const double E1 = eps * E;
   double d1x = t.dx, d1y = t.dy, d1z = t.dz;
-  rotate_dir(d1x, d1y, d1z, cost, sint, 2.0 * kPi * xphi);
+  rotate_dir(d1x, d1y, d1z, cost, sint, 2.0 * xphi);
   const double Te = E - E1;
   if (P.electrons_local || Te < P.cut) {
     edep += Te;
@@ -221,6 +221,7 @@ __device__ __forceinline__ bool compton(const DeviceState& D, uint32_t slot, uin
 }
 
 // S5 photon move: sampled free path vs distance to boundary; returns the next action
+template <int GEOM>
 __device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& eesc) {
   const Params& P = D.P;
   const int vol0 = t.vol;
@@ -241,7 +242,7 @@ __device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, 
   const double x = xi1 * stot;
   const int process = (x < sPE) ? A_PE : ((x < sPE + sPair) ? A_PAIR : A_COMPTON);
   int which;
-  const double s_b = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, which);
+  const double s_b = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, s_d, which);
   if (t.nsteps < 65535u) t.nsteps += 1;
   if (s_d < s_b) {
     t.a.x += s_d * t.dx; t.a.y += s_d * t.dy; t.a.z += s_d * t.dz;
@@ -249,7 +250,7 @@ __device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, 
     return process;
   }
   t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
-  const bool escaped = cross_boundary(P, t.a.z, t.dz, t.vol, t.surf, which);
+  const bool escaped = cross_boundary<GEOM>(P, t.a.z, t.dz, t.vol, t.surf, which);
   if (escaped) {
     eesc += t.a.energy;
     if (t.vol < 0 || t.vol > 254) t.vol = vol0;
@@ -258,6 +259,7 @@ __device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, 
   return A_MOVE_G;
 }
 
+template <int GEOM>
 __global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
   CEL_FOR_RANGE(R_PHOTON) {
     const uint32_t slot = slot_of(D, tid);
@@ -272,13 +274,14 @@ __global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
     int action = A_VACANT;
     bool alive = true;
     if (act == A_COMPTON) alive = compton(D, slot, k_iter, t, edep, nsec);
-    if (alive) action = move_photon(D, slot, k_iter, t, eesc);
+    if (alive) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
     finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
   }
 }
 
 // ================================================================ charged: bremsstrahlung (S8) then move (S7)
 // S7: step limit -> linear or helical propagation (<= max_substeps chord substeps) -> CSDA loss -> MSC -> fate
+template <bool FIELD, int GEOM>
 __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, double& eesc) {
   const Params& P = D.P;
   const int vol0 = t.vol;
@@ -291,8 +294,7 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
     return stop_charged(P, ptype, edep);
   }
   const int mat = __ldg(P.vol_material + t.vol);
-  const double p = sqrt(T0 * (T0 + 2.0 * kElectronMass));
-  const double beta = p / (T0 + kElectronMass);
+  const double p2 = T0 * (T0 + 2.0 * kElectronMass);   // p^2; beta p = p^2 / (T0 + m_e)
   // S7.2 step limit
   double r0 = 0.0, s_r = CEL_INF, s_d = CEL_INF;
   int j0 = 0;
@@ -316,20 +318,20 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
   // S7.3 propagation
   double travelled = 0.0;
   bool escaped = false, complete = false;
-  if (P.bmag == 0.0) {
+  if (!FIELD) {
     int which;
-    const double s_b = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, which);
+    const double s_b = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, s_phys, which);
     if (s_phys < s_b) {
       t.a.x += s_phys * t.dx; t.a.y += s_phys * t.dy; t.a.z += s_phys * t.dz;
       t.surf = -1; travelled = s_phys; complete = true;
     } else {
       t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
       travelled = s_b;
-      escaped = cross_boundary(P, t.a.z, t.dz, t.vol, t.surf, which);
+      escaped = cross_boundary<GEOM>(P, t.a.z, t.dz, t.vol, t.surf, which);
     }
   } else {
     const double q = (ptype == P_ELECTRON) ? -1.0 : 1.0;
-    const double omega = q * kKappa * P.bmag / p;
+    const double omega = q * kKappa * P.bmag / sqrt(p2);
     const double h_max = fmin(sqrt(8.0 * kDeltaChord / fabs(omega)), 0.5 / fabs(omega));
     double remaining = s_phys;
     int n = 0;
@@ -345,7 +347,7 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
         const double cx = nx - t.a.x, cy = ny - t.a.y, cz = nz - t.a.z;
         l = sqrt(cx * cx + cy * cy + cz * cz);
         chx = cx / l; chy = cy / l; chz = cz / l;
-        tb = distance_to_boundary(P, t.a.x, t.a.y, t.a.z, chx, chy, chz, t.vol, t.surf, which);
+        tb = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, chx, chy, chz, t.vol, t.surf, l, which);
         // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
         if (tb == 0.0 && halvings < kMaxDipHalvings &&
             tangent_points_inward(P, t.a.x, t.a.y, t.dx, t.dy, t.dz, chx, chy, chz, which)) { h *= 0.5; continue; }
@@ -359,7 +361,7 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
         normalise3(fdx, fdy, fdz);
         t.dx = fdx; t.dy = fdy; t.dz = fdz;
         travelled += f * h;
-        escaped = cross_boundary(P, t.a.z, chz, t.vol, t.surf, which);
+        escaped = cross_boundary<GEOM>(P, t.a.z, chz, t.vol, t.surf, which);
         break;
       }
       normalise3(ndx, ndy, ndz);
@@ -383,13 +385,13 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
   // S7.5 multiple scattering
   if (P.enable_msc && !escaped && mat >= 0 && travelled > 0.0 && T1 >= P.cut) {
     const double x = travelled * __ldg(&P.mats[mat].inv_X0);
-    const double theta0 = 13.6 / (beta * p) * sqrt(x) * fmax(0.0, 1.0 + 0.038 * log(x));
+    const double theta0 = 13.6 * (T0 + kElectronMass) / p2 * sqrt(x) * fmax(0.0, 1.0 + 0.038 * log(x));
     double xm0, xm1;
     draw_pair(P, slot, k_iter, PH_MSC, 0, xm0, xm1);
     const double theta = fmin(theta0 * sqrt(-2.0 * log(xm0)), kPi);
     double st, ct;
     sincos(theta, &st, &ct);
-    rotate_dir(t.dx, t.dy, t.dz, ct, st, 2.0 * kPi * xm1);
+    rotate_dir(t.dx, t.dy, t.dz, ct, st, 2.0 * xm1);
   }
   // S7.6 fate
   const double rest = (ptype == P_POSITRON) ? 2.0 * kElectronMass : 0.0;
@@ -410,6 +412,7 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
   return (interaction_wins && complete) ? A_BREMS : A_MOVE_C;
 }
 
+template <bool FIELD, int GEOM>
 __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
@@ -431,7 +434,7 @@ __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
       if (T1 < P.cut) { edep += T1; t.a.energy = 0.0; action = stop_charged(P, t.ptype, edep); }
       else t.a.energy = T1;
     }
-    if (action == A_MOVE_C) action = move_charged(D, slot, k_iter, t, edep, eesc);
+    if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
     finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
   }
 }
