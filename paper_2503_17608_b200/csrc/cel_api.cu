@@ -4,6 +4,7 @@
 #include "../../include/cel.h"
 #include "cel_kernels.cuh"
 #include "cel_physics.cuh"
+#include "cel_persistent.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -50,12 +51,16 @@ struct cel_ctx {
   cudaStream_t side[kSideStreams] = {nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
   cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr};
   int concurrent = 1;
+  int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
   Control* h_status = nullptr;      // pinned, kStatusSlots entries
   uint64_t* h_tally = nullptr; size_t h_tally_bytes = 0;   // pinned
   void* h_prim = nullptr; size_t h_prim_bytes = 0;         // pinned staging of primaries
   cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
   int use_graph = 1; int batch = 16; int64_t max_iterations = 1ll << 22;
+  int persistent = 0; int persist_batch = 64;   // one cooperative kernel runs up to persist_batch iterations
+  int persist_grid = 0;                         // co-resident blocks of k_persistent (0 = not available)
+  const void* persist_fn = nullptr;
   int n_sm = 148;
   bool ran = false; int run_error = 0;
   uint64_t launches = 0; int kernels_per_iteration = 0;
@@ -71,6 +76,8 @@ struct cel_ctx {
 };
 
 namespace {
+
+void setup_persistent(cel_ctx* c);   // defined with the host loop below
 
 #define CEL_CUDA(ctx, call)                                                        \
   do {                                                                             \
@@ -319,6 +326,7 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   const Tiling tl = make_tiling(n_slots);
   D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
   D.sort_mode = sort_mode;
+  setup_persistent(c);
   D.init_capacity = default_capacity(n_slots, ph->init_capacity);
 
   if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);
@@ -384,6 +392,9 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "batch")) { if (v < 1 || v > 4096) return CEL_ERR_INVALID_ARG; c->batch = (int)v; }
   else if (!std::strcmp(name, "profile")) c->profile = v ? 1 : 0;
   else if (!std::strcmp(name, "concurrent")) c->concurrent = v ? 1 : 0;
+  else if (!std::strcmp(name, "persistent")) c->persistent = v ? 1 : 0;
+  else if (!std::strcmp(name, "pdl")) c->pdl = v ? 1 : 0;
+  else if (!std::strcmp(name, "persist_batch")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->persist_batch = (int)v; }
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
   return CEL_OK;
@@ -424,6 +435,18 @@ inline void after_launch(cel_ctx* c, int id, int& n) {
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1) + n], c->stream);
 }
 
+// launch on the main-stream chain: with `pdl` the kernel may be scheduled while its predecessor in the stream drains
+template <typename K>
+void launch_chain(cel_ctx* c, K kernel, int grid, int block, cudaStream_t s) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = (c->pdl && !c->profile) ? 1 : 0;
+  cudaLaunchKernelEx(&cfg, kernel, c->D);
+}
+
 // one step iteration = P1, P2, P3 (+P4 inside the action kernels), P5 (docs/PHYSICS_SPEC.md S1); returns the number of
 // kernels enqueued. The five action kernels touch disjoint slots. Sorted by action, their ranges are fixed by the sort,
 // so they are independent and run as parallel branches (side streams; parallel graph branches under capture). In the
@@ -437,8 +460,8 @@ int enqueue_iteration(cel_ctx* c) {
   const bool fork = c->concurrent && !c->profile;
   int n = 0;
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1)], s);
-  k_init_fill<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_INIT_FILL, n);
-  if (D.sort_mode != CEL_SORT_NONE) { k_scatter<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_SCATTER, n); }
+  launch_chain(c, k_init_fill, tg, kTileThreads, s); after_launch(c, CEL_K_INIT_FILL, n);
+  if (D.sort_mode != CEL_SORT_NONE) { launch_chain(c, k_scatter, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n); }
   cudaStream_t s_photon = s, s_small = s;
   if (fork) {
     cudaEventRecord(c->ev_fork, s);
@@ -454,8 +477,9 @@ int enqueue_iteration(cel_ctx* c) {
   const bool cyl = D.P.geom_kind == CEL_GEOM_CYL, field = D.P.bmag != 0.0;
   if (cyl) k_photon<1><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0><<<pg, kBlock, 0, s_photon>>>(D);
   after_launch(c, CEL_K_PHOTON, n);
-  if (cyl) { if (field) k_charged<true, 1><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 1><<<pg, kBlock, 0, s>>>(D); }
-  else { if (field) k_charged<true, 0><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0><<<pg, kBlock, 0, s>>>(D); }
+  // (in the masked modes the annihilation kernel precedes it on the main stream)
+  if (cyl) { if (field) launch_chain(c, k_charged<true, 1>, pg, kBlock, s); else launch_chain(c, k_charged<false, 1>, pg, kBlock, s); }
+  else { if (field) launch_chain(c, k_charged<true, 0>, pg, kBlock, s); else launch_chain(c, k_charged<false, 0>, pg, kBlock, s); }
   after_launch(c, CEL_K_CHARGED, n);
   if (fork) {
     cudaEventRecord(c->ev_join[0], c->side[0]);
@@ -465,7 +489,7 @@ int enqueue_iteration(cel_ctx* c) {
       cudaStreamWaitEvent(s, c->ev_join[1], 0);
     }
   }
-  k_push<<<tg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_PUSH, n);
+  launch_chain(c, k_push, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
   return n;
 }
 
@@ -483,10 +507,39 @@ int collect_profile(cel_ctx* c, int n_iter, int kernels_per_iteration) {
   return CEL_OK;
 }
 
+// ---- the persistent form (cel_persistent.cuh): one cooperative kernel per batch of iterations
+const void* persistent_function(const cel_ctx* c) {
+  const bool cyl = c->D.P.geom_kind == CEL_GEOM_CYL, field = c->D.P.bmag != 0.0;
+  if (cyl) return field ? (const void*)k_persistent<true, 1> : (const void*)k_persistent<false, 1>;
+  return field ? (const void*)k_persistent<true, 0> : (const void*)k_persistent<false, 0>;
+}
+// co-resident grid for the cooperative launch; 0 if the device cannot run it (then the kernel-per-action form is used)
+void setup_persistent(cel_ctx* c) {
+  c->persist_fn = persistent_function(c);
+  c->persist_grid = 0;
+  int dev = 0, coop = 0, per_sm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return;
+  if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, c->persist_fn, kTileThreads, 0) != cudaSuccess || per_sm < 1) return;
+  const int grid = per_sm * c->n_sm;
+  if ((c->D.n_tiles + grid - 1) / grid > (uint32_t)kMaxTilesPerBlock) return;
+  c->persist_grid = grid;
+}
+bool use_persistent(const cel_ctx* c) { return c->persistent && !c->profile && c->persist_grid > 0; }
+int launch_persistent(cel_ctx* c, uint32_t max_iters) {
+  CEL_CUDA(c, cudaMemsetAsync(&c->D.ctl->barrier, 0, sizeof(unsigned long long), c->stream));
+  DeviceState D = c->D;
+  void* args[] = {(void*)&D, (void*)&max_iters};
+  CEL_CUDA(c, cudaLaunchCooperativeKernel(c->persist_fn, dim3(c->persist_grid), dim3(kTileThreads), args, 0, c->stream));
+  c->launches += 1;
+  return CEL_OK;
+}
+
 // reset slots, staging, counters and tallies; allocate the run's scratch with the stream-ordered allocator
-int prepare_run(cel_ctx* c, uint32_t n_events) {
+int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   int rc = lay_out(c);
   if (rc != CEL_OK) return rc;
+  c->D.write_vacant = debug ? 1 : 0;   // the complete permutation is only needed by the parity surface
   cudaStream_t s = c->stream;
   DeviceState& D = c->D;
   // stream-ordered scratch: freed and re-allocated on the stream, never a device-wide sync
@@ -527,9 +580,10 @@ int prepare_run(cel_ctx* c, uint32_t n_events) {
       c->prof_ev.push_back(e);
     }
   }
-  if (c->use_graph && !c->profile) {
+  if (c->use_graph && !c->profile && !use_persistent(c)) {
+    // one graph = one batch of iterations: a single cudaGraphLaunch per status poll keeps the host far ahead of the device
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
-    c->kernels_per_iteration = enqueue_iteration(c);
+    for (int b = 0; b < c->batch; ++b) c->kernels_per_iteration = enqueue_iteration(c);
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
     CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
   }
@@ -583,10 +637,18 @@ int run_loop(cel_ctx* c) {
   int rc = CEL_OK;
   while (true) {
     int per_iter = c->kernels_per_iteration;
-    for (int b = 0; b < c->batch; ++b) {
-      c->prof_b = b;
-      if (c->graph_exec) { CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s)); c->launches += c->kernels_per_iteration; }
-      else { per_iter = enqueue_iteration(c); c->launches += per_iter; }
+    if (use_persistent(c)) {
+      int prc = launch_persistent(c, (uint32_t)c->persist_batch);
+      if (prc != CEL_OK) return prc;
+      enqueued += c->persist_batch - c->batch;
+    } else if (c->graph_exec) {
+      CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s));
+      c->launches += (uint64_t)c->kernels_per_iteration * c->batch;
+    } else {
+      for (int b = 0; b < c->batch; ++b) {
+        c->prof_b = b;
+        per_iter = enqueue_iteration(c); c->launches += per_iter;
+      }
     }
     c->prof_b = 0;
     enqueued += c->batch;
@@ -616,14 +678,14 @@ extern "C" int cel_transport(cel_ctx* c, const cel_primary* primaries, uint64_t 
   if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
   int rc = validate_primaries(c, primaries, n, n_events);
   if (rc != CEL_OK) return rc;
-  if ((rc = prepare_run(c, n_events)) != CEL_OK) return rc;
+  if ((rc = prepare_run(c, n_events, false)) != CEL_OK) return rc;
   if ((rc = load_primaries_host(c, primaries, n)) != CEL_OK) return rc;
   return run_loop(c);
 }
 
 extern "C" int cel_transport_device(cel_ctx* c, const void* d_primaries, uint64_t n, uint32_t n_events) {
   if (!c || (!d_primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
-  int rc = prepare_run(c, n_events);
+  int rc = prepare_run(c, n_events, false);
   if (rc != CEL_OK) return rc;
   k_load_primaries<<<c->n_sm, 256, 0, c->stream>>>(c->D, (const PrimaryRec*)d_primaries, n);
   c->launches += 1;
@@ -664,7 +726,7 @@ extern "C" int cel_debug_begin(cel_ctx* c, const cel_primary* primaries, uint64_
   if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
   int rc = validate_primaries(c, primaries, n, n_events);
   if (rc != CEL_OK) return rc;
-  if ((rc = prepare_run(c, n_events)) != CEL_OK) return rc;
+  if ((rc = prepare_run(c, n_events, true)) != CEL_OK) return rc;
   if ((rc = load_primaries_host(c, primaries, n)) != CEL_OK) return rc;
   CEL_CUDA(c, cudaEventRecord(c->ev_start, c->stream));
   CEL_CUDA(c, cudaEventRecord(c->ev_stop, c->stream));
@@ -674,7 +736,8 @@ extern "C" int cel_debug_begin(cel_ctx* c, const cel_primary* primaries, uint64_
 
 extern "C" int cel_debug_step(cel_ctx* c) {
   if (!c || !c->ran) return CEL_ERR_NOT_RUN;
-  c->launches += enqueue_iteration(c);
+  if (use_persistent(c)) { int prc = launch_persistent(c, 1); if (prc != CEL_OK) return prc; }
+  else c->launches += enqueue_iteration(c);
   CEL_CUDA(c, cudaGetLastError());
   CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[0], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
   CEL_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -117,6 +117,7 @@ struct Control {
   uint32_t ticket_fill, ticket_push;
   uint32_t n_logged;
   uint32_t vac_total;               // V before the fill of this iteration
+  unsigned long long barrier;       // arrival counter of the persistent kernel's grid barrier (zeroed per launch)
 };
 
 // everything a kernel needs; passed by value (fits in the 4 KB parameter space)
@@ -127,6 +128,7 @@ struct DeviceState {
   uint32_t tile_shift;    // log2(tile_slots)
   uint32_t subs_per_tile; // tile_slots / kSub
   int sort_mode;
+  int write_vacant;       // 1 = also write the indices of vacant slots (complete permutation, debug surface)
   unsigned long long init_capacity;
   uint32_t n_events;
   uint32_t log_capacity;
@@ -144,6 +146,16 @@ struct DeviceState {
   uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
   uint32_t* tile_hist;    // [n_tiles][8] per-tile sort-key histogram -> exclusive base per key after k_init_fill
 };
+
+// ---------------------------------------------------------------- programmatic dependent launch (sm_90+)
+// The kernels of the main-stream chain (fill -> scatter -> charged -> push -> next fill) are launched with the
+// programmatic-stream-serialization attribute: a kernel lets its successor's blocks be scheduled early
+// (launch_dependents) and waits itself, before touching any memory, until its predecessors have completed and
+// flushed (wait). Without the attribute both instructions are no-ops.
+__device__ __forceinline__ void pdl_prologue() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
 
 // ---------------------------------------------------------------- S3 Philox4x32-10
 struct Philox4 { uint32_t w[4]; };

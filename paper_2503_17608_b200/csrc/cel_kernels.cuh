@@ -126,28 +126,35 @@ __device__ __forceinline__ uint32_t count_vacant4(uint32_t w) {
   return __popc(z);
 }
 
+// ---------------------------------------------------------------- shared memory of a bookkeeping block
+struct BookSmem {
+  uint32_t scan[18];
+  unsigned long long scan64[9];
+  uint32_t hist[8], act[8], base[8];
+  uint32_t skey[kTileThreads];   // the sub-tile's key bytes
+  uint32_t list[2 * kSub];       // compacted work list of the cooperative copies
+};
+
+__device__ __forceinline__ uint32_t real_slots_in_tile(const DeviceState& D, uint32_t tile) {
+  const unsigned long long lo = (unsigned long long)tile << D.tile_shift, hi = lo + (1ull << D.tile_shift);
+  return lo >= D.N ? 0u : (uint32_t)((hi < D.N ? hi : (unsigned long long)D.N) - lo);
+}
+
 // ================================================================ P1: vacancy scan + fill (S9), P2 histogram (S2)
 // Rank-r vacant slot (ascending slot order) takes init[I-1-r] when r < I (LIFO). The rank of a tile's first vacancy
-// is the sum of tile_vac over the tiles before it — scan-based, no atomics in the assignment, so the slot assignment
-// is deterministic. The kernel also builds the per-tile histogram of sort keys for P2 and, in its last
-// block, the key offsets, the action kernels' ranges, the counters and the per-iteration log.
-__global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
-  __shared__ uint32_t smem[18];
-  __shared__ uint32_t hist_s[8], act_s[8];
-  __shared__ uint32_t skey[kTileThreads];   // the sub-tile's key bytes
-  __shared__ uint32_t list[kSub];           // slots to fill, by rank inside the sub-tile
-  Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const uint32_t tile = blockIdx.x;
-  const unsigned long long I = ctl->n_init;
-  if (threadIdx.x < 8) { hist_s[threadIdx.x] = 0; act_s[threadIdx.x] = 0; }
-  uint32_t prefix, V;
-  block_prefix_total(D.tile_vac, D.n_tiles, tile, smem, prefix, V);   // (its barriers also publish hist_s / act_s)
-  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
-  const uint32_t tile_vacant = D.tile_vac[tile];
+// (`prefix`) is the sum of tile_vac over the tiles before it — scan-based, no atomics in the assignment, so the slot
+// assignment is deterministic. Adds the tile's action histogram to sm.act and (sort by particle) its
+// sort-key histogram to sm.hist; the caller zeroes both and synchronises before, and synchronises after.
+__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t n_take,
+                                          uint32_t prefix, uint32_t tile_vacant) {
   uint32_t rank0 = prefix;                                   // rank of the first vacancy of the current sub-tile
   const uint32_t rank_end = prefix + tile_vacant;            // one past the rank of the tile's last vacancy
-  uint8_t* skey_b = reinterpret_cast<uint8_t*>(skey);
+  const uint32_t real = real_slots_in_tile(D, tile);
+  if (tile_vacant == real && !(prefix < n_take)) {           // all vacant, nothing to fill: no key byte needs reading
+    if (threadIdx.x == 0) { atomicAdd(&sm.act[A_VACANT], real); if (D.sort_mode == 2) atomicAdd(&sm.hist[3], real); }
+    return;
+  }
+  uint8_t* skey_b = reinterpret_cast<uint8_t*>(sm.skey);
   for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
     const uint32_t sub_base = (tile << D.tile_shift) + sub * kSub;
     const uint32_t base = sub_base + threadIdx.x * kKeysPerThread;
@@ -155,19 +162,19 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
     if (rank0 < n_take && rank0 < rank_end) {               // block-uniform: this sub-tile may have vacancies to fill
       const uint32_t c = count_vacant4(kv);
       uint32_t total;
-      uint32_t r = block_excl_scan(c, smem, total);
-      skey[threadIdx.x] = kv;
+      uint32_t r = block_excl_scan(c, sm.scan, total);
+      sm.skey[threadIdx.x] = kv;
       if (c) {
 #pragma unroll
         for (int i = 0; i < kKeysPerThread; ++i)
-          if (((kv >> (8 * i)) & 0xf) == A_VACANT) { list[r] = base + i; ++r; }
+          if (((kv >> (8 * i)) & 0xf) == A_VACANT) { sm.list[r] = base + i; ++r; }
       }
       __syncthreads();
       const uint32_t nf = min(total, n_take - rank0);
       // cooperative copy: work item w = (record, half); half 0 = RecA, half 1 = RecB (+ the key byte)
       for (uint32_t w = threadIdx.x; w < 2 * nf; w += kTileThreads) {
         const uint32_t item = w >> 1;
-        const uint32_t slot = list[item];
+        const uint32_t slot = sm.list[item];
         const unsigned long long src = I - 1ull - (unsigned long long)(rank0 + item);
         if (w & 1) {
           const RecB b = load_b(D.initB + src);
@@ -180,7 +187,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
         }
       }
       __syncthreads();
-      kv = skey[threadIdx.x];
+      kv = sm.skey[threadIdx.x];
       rank0 += total;
     }
     // histograms of this thread's 4 keys, 8 x 8-bit packed (padding bytes 0xff are skipped)
@@ -201,42 +208,193 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
         const uint32_t lo = (a_lo >> (8 * a)) & 0xff, hi = (a_hi >> (8 * a)) & 0xff;
-        if (lo) atomicAdd(&act_s[a], lo);
-        if (hi) atomicAdd(&act_s[a + 4], hi);
-        if (D.sort_mode == 2) { const uint32_t s = (s_lo >> (8 * a)) & 0xff; if (s) atomicAdd(&hist_s[a], s); }
+        if (lo) atomicAdd(&sm.act[a], lo);
+        if (hi) atomicAdd(&sm.act[a + 4], hi);
+        if (D.sort_mode == 2) { const uint32_t h = (s_lo >> (8 * a)) & 0xff; if (h) atomicAdd(&sm.hist[a], h); }
       }
     }
   }
-  __syncthreads();
+}
+// after fill_tile + __syncthreads: publish the tile's sort-key histogram and add its action counts to the iteration's
+__device__ __forceinline__ void publish_tile_hist(const DeviceState& D, BookSmem& sm, uint32_t tile) {
   if (threadIdx.x < 8) {
-    const uint32_t a = act_s[threadIdx.x];
-    D.tile_hist[tile * 8 + threadIdx.x] = (D.sort_mode == 2) ? hist_s[threadIdx.x] : a;
-    if (a) atomicAdd(&ctl->counts_acc[threadIdx.x], a);
+    const uint32_t a = sm.act[threadIdx.x];
+    D.tile_hist[tile * 8 + threadIdx.x] = (D.sort_mode == 2) ? sm.hist[threadIdx.x] : a;
+    if (a) atomicAdd(&D.ctl->counts_acc[threadIdx.x], a);
   }
+}
+// vacancies of a tile that the fill of this iteration takes: min(v, max(0, n_take - (vacancies before the tile)))
+__device__ __forceinline__ uint32_t filled_in_tile(uint32_t v, uint32_t prefix, uint32_t n_take) {
+  return min(v, n_take > prefix ? n_take - prefix : 0u);
+}
+
+// ================================================================ P2: stable scatter of slot indices (S2)
+// indices[offset[key] + (tiles before)[key] + (rank inside the tile)] = slot; ascending slot order inside a key.
+// The caller sets sm.base[key] = offset[key] + (tiles before)[key] and synchronises. Vacant slots are never launched:
+// their indices are written only when the complete permutation is asked for (debug surface), and a tile that is
+// entirely vacant is then skipped without reading its key bytes.
+__device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, uint32_t tile_vacant_now) {
+  const int vacant_key = D.sort_mode == 1 ? (int)A_VACANT : 3;
+  if (!D.write_vacant && tile_vacant_now == real_slots_in_tile(D, tile)) return;
+  for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
+    const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
+    const uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
+    // per-thread key counts, 4 x 16-bit packed in two words (keys 0-3, 4-7); a sub-tile has 1024 slots < 2^16
+    unsigned long long lo = 0, hi = 0;
+#pragma unroll
+    for (int i = 0; i < kKeysPerThread; ++i) {
+      const uint32_t kb = (kv >> (8 * i)) & 0xff;
+      if (kb != 0xff) {
+        const int s = sort_key_of(D.sort_mode, kb);
+        if (s < 4) lo += 1ull << (16 * s); else hi += 1ull << (16 * (s - 4));
+      }
+    }
+    unsigned long long tot_lo, tot_hi = 0;
+    unsigned long long plo = block_excl_scan64(lo, sm.scan64, tot_lo);
+    unsigned long long phi = 0;
+    if (D.sort_mode == 1) phi = block_excl_scan64(hi, sm.scan64, tot_hi);
+#pragma unroll
+    for (int i = 0; i < kKeysPerThread; ++i) {
+      const uint32_t kb = (kv >> (8 * i)) & 0xff;
+      if (kb != 0xff) {
+        const int s = sort_key_of(D.sort_mode, kb);
+        uint32_t r;
+        if (s < 4) { r = (uint32_t)((plo >> (16 * s)) & 0xffff); plo += 1ull << (16 * s); }
+        else { r = (uint32_t)((phi >> (16 * (s - 4))) & 0xffff); phi += 1ull << (16 * (s - 4)); }
+        if (s != vacant_key || D.write_vacant) D.indices[sm.base[s] + r] = base + i;
+      }
+    }
+    if (sub + 1 < D.subs_per_tile) {   // advance the per-key bases by this sub-tile's totals
+      __syncthreads();
+      if (threadIdx.x < 4) sm.base[threadIdx.x] += (uint32_t)((tot_lo >> (16 * threadIdx.x)) & 0xffff);
+      else if (threadIdx.x < 8) sm.base[threadIdx.x] += (uint32_t)((tot_hi >> (16 * (threadIdx.x - 4))) & 0xffff);
+      __syncthreads();
+    }
+  }
+}
+
+// ================================================================ P5: secondary push (S9)
+// Exclusive scan of nsec[slot] in ascending SLOT order (in every sort mode), so that the initializer order — and with
+// it every later slot assignment and PRNG stream — does not depend on thread timing or on the sort mode. A tile's
+// offset `off0` is the sum of tile_sec over the tiles before it; a tile that staged nothing is not read at all.
+__device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t off0,
+                                          uint32_t tile_total, bool overflow) {
+  const uint32_t off_end = off0 + tile_total;
+  for (uint32_t sub = 0; sub < D.subs_per_tile && off0 < off_end; ++sub) {
+    const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
+    const uint32_t nv = *reinterpret_cast<const uint32_t*>(D.nsec + base);
+    const uint32_t c = (nv & 0xff) + ((nv >> 8) & 0xff) + ((nv >> 16) & 0xff) + (nv >> 24);   // bytes are 0..2
+    uint32_t total;
+    uint32_t r = block_excl_scan(c, sm.scan, total);
+    if (c) {
+#pragma unroll
+      for (int i = 0; i < kKeysPerThread; ++i) {
+        const uint32_t n = (nv >> (8 * i)) & 0xff;
+        for (uint32_t j = 0; j < n; ++j) sm.list[r++] = 2u * (base + i) + j;
+      }
+      *reinterpret_cast<uint32_t*>(D.nsec + base) = 0u;   // consumed
+    }
+    __syncthreads();
+    if (!overflow) {
+      for (uint32_t w = threadIdx.x; w < 2 * total; w += kTileThreads) {
+        const uint32_t item = w >> 1;
+        const uint32_t src = sm.list[item];
+        const unsigned long long dst = I + (unsigned long long)(off0 + item);
+        if (w & 1) store_b(D.initB + dst, load_b(D.secB + src));
+        else store_a(D.initA + dst, load_a(D.secA + src));
+      }
+    }
+    off0 += total;
+  }
+}
+
+// S2: the index range of each action kernel from the key offsets
+__device__ __forceinline__ void set_ranges(const DeviceState& D, const uint32_t* off, uint32_t* rb, uint32_t* re) {
+  if (D.sort_mode == 1) {        // PE | PAIR | COMPTON MOVE_G | MOVE_C BREMS | ANNIH | VACANT
+    rb[R_PE] = off[0]; re[R_PE] = off[1];
+    rb[R_PAIR] = off[1]; re[R_PAIR] = off[2];
+    rb[R_PHOTON] = off[2]; re[R_PHOTON] = off[4];
+    rb[R_CHARGED] = off[4]; re[R_CHARGED] = off[6];
+    rb[R_ANNIH] = off[6]; re[R_ANNIH] = off[7];
+  } else if (D.sort_mode == 2) { // gamma | e- | e+ | vacant
+    rb[R_PE] = rb[R_PAIR] = rb[R_PHOTON] = off[0];
+    re[R_PE] = re[R_PAIR] = re[R_PHOTON] = off[1];
+    rb[R_CHARGED] = off[1]; re[R_CHARGED] = off[3];
+    rb[R_ANNIH] = off[2]; re[R_ANNIH] = off[3];
+  } else {
+    for (int k = 0; k < R_COUNT; ++k) { rb[k] = 0; re[k] = D.N; }
+  }
+}
+// end-of-P1 bookkeeping of the control block by one thread (S11): counts, offsets, ranges, I, alive, log
+__device__ __forceinline__ void update_control_after_fill(const DeviceState& D, const uint32_t* key_total, int n_keys,
+                                                          unsigned long long I, uint32_t V, uint32_t n_take) {
+  Control* ctl = D.ctl;
+  uint32_t cnt[8];
+  for (int a = 0; a < 8; ++a) { cnt[a] = ctl->counts_acc[a]; ctl->counts[a] = cnt[a]; ctl->counts_acc[a] = 0; }
+  const uint32_t N = D.N;
+  uint32_t off[9];
+  off[0] = 0;
+  for (int k = 0; k < 8; ++k) off[k + 1] = (k < n_keys) ? off[k] + key_total[k] : off[k];
+  if (n_keys == 0) for (int k = 1; k <= 8; ++k) off[k] = N;
+  for (int k = 0; k <= 8; ++k) ctl->offsets[k] = off[k];
+  set_ranges(D, off, ctl->rb, ctl->re);
+  const uint32_t alive = N - cnt[A_VACANT];
+  const unsigned long long Iafter = I - n_take;   // I -= min(V, I)
+  ctl->vac_total = V;
+  ctl->n_init = Iafter;
+  ctl->alive = alive;
+  if (alive == 0 && Iafter == 0) {
+    ctl->finished = 1;
+  } else {
+    ctl->track_steps += alive;
+    ctl->iterations += 1;
+    const uint32_t k = ctl->n_logged;
+    if (k < D.log_capacity) {
+      for (int a = 0; a < 8; ++a) D.counts_log[(size_t)k * 8 + a] = cnt[a];
+      ctl->n_logged = k + 1;
+    }
+  }
+}
+
+// ================================================================ the bookkeeping kernels (one block per tile)
+// k_init_fill: P1 + the per-tile histograms; its last block turns the histograms into per-key bases (exclusive scan
+// over the tiles), takes the filled vacancies off tile_vac, and updates offsets, ranges, counters and the log.
+__global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
+  __shared__ BookSmem sm;
+  pdl_prologue();
+  Control* ctl = D.ctl;
+  if (ctl->finished) return;
+  const uint32_t tile = blockIdx.x;
+  const unsigned long long I = ctl->n_init;
+  if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
+  uint32_t prefix, V;
+  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);   // (its barriers also publish sm.hist / sm.act)
+  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
+  fill_tile(D, sm, tile, I, n_take, prefix, D.tile_vac[tile]);
+  __syncthreads();
+  publish_tile_hist(D, sm, tile);
   if (!last_block_done(&ctl->ticket_fill)) return;
-  // ---- last block: vacancies left per tile, per-key exclusive scan over tiles, offsets, ranges, counters
-  {  // tile t keeps v - (filled in t), filled = min(v, max(0, n_take - (vacancies before t))); thread owns `per` tiles
-    const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;
-    const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
+  // ---- last block: thread t owns `per` consecutive tiles
+  const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;   // <= kMaxTiles / 256 = 8
+  const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
+  {  // vacancies left per tile
     uint32_t v[kMaxTiles / kTileThreads];
     uint32_t sum = 0;
 #pragma unroll
     for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) { v[i] = (t0 + i < t1) ? D.tile_vac[t0 + i] : 0; sum += v[i]; }
     uint32_t total;
-    uint32_t ex = block_excl_scan(sum, smem, total);
+    uint32_t ex = block_excl_scan(sum, sm.scan, total);
 #pragma unroll
     for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) {
-      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - min(v[i], n_take > ex ? n_take - ex : 0u);
+      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - filled_in_tile(v[i], ex, n_take);
       ex += v[i];
     }
   }
-  // per-key exclusive scan of tile_hist over the tiles, all keys in one pass: thread t owns `per` consecutive tiles
+  // per-key exclusive scan of tile_hist over the tiles, all keys in one pass
   __shared__ uint32_t key_total[8];
   __shared__ uint32_t warp_tot[kTileThreads / 32][8];
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
   if (n_keys) {
-    const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;   // <= kMaxTiles / 256 = 8
-    const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
     uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     for (uint32_t t = t0; t < t1; ++t) {
       const uint4 a = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8), b = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8 + 4);
@@ -267,139 +425,31 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
     }
     __syncthreads();
   }
-  if (threadIdx.x == 0) {
-    uint32_t cnt[8];
-    for (int a = 0; a < 8; ++a) { cnt[a] = ctl->counts_acc[a]; ctl->counts[a] = cnt[a]; ctl->counts_acc[a] = 0; }
-    const uint32_t N = D.N;
-    uint32_t off[9];
-    off[0] = 0;
-    for (int k = 0; k < 8; ++k) off[k + 1] = (k < n_keys) ? off[k] + key_total[k] : off[k];
-    if (n_keys == 0) for (int k = 1; k <= 8; ++k) off[k] = N;
-    for (int k = 0; k <= 8; ++k) ctl->offsets[k] = off[k];
-    uint32_t* rb = ctl->rb; uint32_t* re = ctl->re;
-    if (D.sort_mode == 1) {        // S2: PE | PAIR | COMPTON MOVE_G | MOVE_C BREMS | ANNIH | VACANT
-      rb[R_PE] = off[0]; re[R_PE] = off[1];
-      rb[R_PAIR] = off[1]; re[R_PAIR] = off[2];
-      rb[R_PHOTON] = off[2]; re[R_PHOTON] = off[4];
-      rb[R_CHARGED] = off[4]; re[R_CHARGED] = off[6];
-      rb[R_ANNIH] = off[6]; re[R_ANNIH] = off[7];
-    } else if (D.sort_mode == 2) { // gamma | e- | e+ | vacant
-      rb[R_PE] = rb[R_PAIR] = rb[R_PHOTON] = off[0];
-      re[R_PE] = re[R_PAIR] = re[R_PHOTON] = off[1];
-      rb[R_CHARGED] = off[1]; re[R_CHARGED] = off[3];
-      rb[R_ANNIH] = off[2]; re[R_ANNIH] = off[3];
-    } else {
-      for (int k = 0; k < R_COUNT; ++k) { rb[k] = 0; re[k] = N; }
-    }
-    const uint32_t alive = N - cnt[A_VACANT];
-    const unsigned long long Iafter = I - n_take;   // I -= min(V, I)
-    ctl->vac_total = V;
-    ctl->n_init = Iafter;
-    ctl->alive = alive;
-    if (alive == 0 && Iafter == 0) {
-      ctl->finished = 1;
-    } else {
-      ctl->track_steps += alive;
-      ctl->iterations += 1;
-      const uint32_t k = ctl->n_logged;
-      if (k < D.log_capacity) {
-        for (int a = 0; a < 8; ++a) D.counts_log[(size_t)k * 8 + a] = cnt[a];
-        ctl->n_logged = k + 1;
-      }
-    }
-  }
+  if (threadIdx.x == 0) update_control_after_fill(D, key_total, n_keys, I, V, n_take);
 }
 
-// ================================================================ P2: stable scatter of slot indices (S2)
-// indices[offset[key] + (tiles before)[key] + (rank inside the tile)] = slot; ascending slot order inside a key.
-// Vacant slots are never launched; their indices are still written so that the permutation is complete.
 __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
-  __shared__ unsigned long long smem64[9];
-  __shared__ uint32_t base_s[8];
-  Control* ctl = D.ctl;
+  __shared__ BookSmem sm;
+  pdl_prologue();
+  const Control* ctl = D.ctl;
   if (ctl->finished) return;
   const uint32_t tile = blockIdx.x;
-  if (threadIdx.x < 8) base_s[threadIdx.x] = ctl->offsets[threadIdx.x] + D.tile_hist[tile * 8 + threadIdx.x];
-  for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
-    const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
-    const uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
-    // per-thread key counts, 4 x 16-bit packed in two words (keys 0-3, 4-7); a sub-tile has 1024 slots < 2^16
-    unsigned long long lo = 0, hi = 0;
-#pragma unroll
-    for (int i = 0; i < kKeysPerThread; ++i) {
-      const uint32_t kb = (kv >> (8 * i)) & 0xff;
-      if (kb != 0xff) {
-        const int s = sort_key_of(D.sort_mode, kb);
-        if (s < 4) lo += 1ull << (16 * s); else hi += 1ull << (16 * (s - 4));
-      }
-    }
-    unsigned long long tot_lo, tot_hi = 0;
-    unsigned long long plo = block_excl_scan64(lo, smem64, tot_lo);
-    unsigned long long phi = 0;
-    if (D.sort_mode == 1) phi = block_excl_scan64(hi, smem64, tot_hi);
-#pragma unroll
-    for (int i = 0; i < kKeysPerThread; ++i) {
-      const uint32_t kb = (kv >> (8 * i)) & 0xff;
-      if (kb != 0xff) {
-        const int s = sort_key_of(D.sort_mode, kb);
-        uint32_t r;
-        if (s < 4) { r = (uint32_t)((plo >> (16 * s)) & 0xffff); plo += 1ull << (16 * s); }
-        else { r = (uint32_t)((phi >> (16 * (s - 4))) & 0xffff); phi += 1ull << (16 * (s - 4)); }
-        D.indices[base_s[s] + r] = base + i;
-      }
-    }
-    if (sub + 1 < D.subs_per_tile) {   // advance the per-key bases by this sub-tile's totals
-      __syncthreads();
-      if (threadIdx.x < 4) base_s[threadIdx.x] += (uint32_t)((tot_lo >> (16 * threadIdx.x)) & 0xffff);
-      else if (threadIdx.x < 8) base_s[threadIdx.x] += (uint32_t)((tot_hi >> (16 * (threadIdx.x - 4))) & 0xffff);
-      __syncthreads();
-    }
-  }
+  if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + D.tile_hist[tile * 8 + threadIdx.x];
+  __syncthreads();
+  scatter_tile(D, sm, tile, D.tile_vac[tile]);
 }
 
-// ================================================================ P5: secondary push (S9)
-// Exclusive scan of nsec[slot] in ascending SLOT order (in every sort mode), so that the initializer order — and with
-// it every later slot assignment and PRNG stream — does not depend on thread timing or on the sort mode. A tile's
-// offset is the sum of tile_sec over the tiles before it; tiles that staged nothing skip their dense bytes.
 __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
-  __shared__ uint32_t smem[18];
-  __shared__ uint32_t list[2 * kSub];       // staged record index (2 * slot + j), by push order inside the sub-tile
+  __shared__ BookSmem sm;
+  pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
   uint32_t prefix, S;
-  block_prefix_total(D.tile_sec, D.n_tiles, tile, smem, prefix, S);
+  block_prefix_total(D.tile_sec, D.n_tiles, tile, sm.scan, prefix, S);
   const bool overflow = ctl->error != 0 || I + S > D.init_capacity;
-  const uint32_t tile_total = D.tile_sec[tile];
-  uint32_t off0 = prefix;
-  const uint32_t off_end = prefix + tile_total;
-  for (uint32_t sub = 0; sub < D.subs_per_tile && off0 < off_end; ++sub) {
-    const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
-    const uint32_t nv = *reinterpret_cast<const uint32_t*>(D.nsec + base);
-    const uint32_t c = (nv & 0xff) + ((nv >> 8) & 0xff) + ((nv >> 16) & 0xff) + (nv >> 24);   // bytes are 0..2
-    uint32_t total;
-    uint32_t r = block_excl_scan(c, smem, total);
-    if (c) {
-#pragma unroll
-      for (int i = 0; i < kKeysPerThread; ++i) {
-        const uint32_t n = (nv >> (8 * i)) & 0xff;
-        for (uint32_t j = 0; j < n; ++j) list[r++] = 2u * (base + i) + j;
-      }
-      *reinterpret_cast<uint32_t*>(D.nsec + base) = 0u;   // consumed
-    }
-    __syncthreads();
-    if (!overflow) {
-      for (uint32_t w = threadIdx.x; w < 2 * total; w += kTileThreads) {
-        const uint32_t item = w >> 1;
-        const uint32_t src = list[item];
-        const unsigned long long dst = I + (unsigned long long)(off0 + item);
-        if (w & 1) store_b(D.initB + dst, load_b(D.secB + src));
-        else store_a(D.initA + dst, load_a(D.secA + src));
-      }
-    }
-    off0 += total;
-  }
+  push_tile(D, sm, tile, I, prefix, D.tile_sec[tile], overflow);
   if (last_block_done(&ctl->ticket_push)) {
     for (uint32_t i = threadIdx.x; i < D.n_tiles; i += kTileThreads) D.tile_sec[i] = 0;
     if (threadIdx.x == 0) {

@@ -112,6 +112,7 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 // ================================================================ P3i: pure interactions (the slot is vacated)
 // Loop over the kernel's index range with a grid-stride loop; `slot` is the gathered slot index.
 #define CEL_FOR_RANGE(RANGE_ID)                                                                             \
+  pdl_prologue();                                                                                           \
   const Control* ctl = D.ctl;                                                                               \
   if (ctl->finished) return;                                                                                \
   const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
@@ -123,61 +124,74 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 __device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode != 0) ? D.indices[tid] : tid; }
 
 // S8 photoelectric: the photon's energy goes to an electron along d (or is deposited when electrons are local)
+__device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t slot, const RecA& a, const RecB& b) {
+  Track t = unpack(a, b);
+  double edep = 0.0;
+  int nsec = 0;
+  if (D.P.electrons_local) edep += t.a.energy;
+  else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
+  finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+}
 __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
   CEL_FOR_RANGE(R_PE) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PE) continue;
     const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     if (meta_action(b.meta) != A_PE) continue;
-    Track t = unpack(load_a(D.stA + slot), b);
-    double edep = 0.0;
-    int nsec = 0;
-    if (P.electrons_local) edep += t.a.energy;
-    else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
-    finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+    do_photoelectric(D, slot, a, b);
   }
 }
 
 // S8 pair: uniform sharing of E - 2 m_e, both collinear; staging order e-, e+
+__device__ __forceinline__ void do_pair(const DeviceState& D, uint32_t slot, uint32_t k_iter, const RecA& a, const RecB& b) {
+  const Params& P = D.P;
+  Track t = unpack(a, b);
+  double edep = 0.0;
+  int nsec = 0;
+  double xi0, xi1;
+  draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+  const double Tav = t.a.energy - 2.0 * kElectronMass;
+  const double Tm = xi0 * Tav;
+  const double Tp = Tav - Tm;
+  if (Tm >= P.cut) stage_secondary(D, slot, nsec++, t, Tm, t.dx, t.dy, t.dz, P_ELECTRON);
+  else edep += Tm;
+  stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
+  finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+}
 __global__ void __launch_bounds__(kBlock) k_pair(DeviceState D) {
   CEL_FOR_RANGE(R_PAIR) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PAIR) continue;
     const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     if (meta_action(b.meta) != A_PAIR) continue;
-    Track t = unpack(load_a(D.stA + slot), b);
-    double edep = 0.0;
-    int nsec = 0;
-    double xi0, xi1;
-    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
-    const double Tav = t.a.energy - 2.0 * kElectronMass;
-    const double Tm = xi0 * Tav;
-    const double Tp = Tav - Tm;
-    if (Tm >= P.cut) stage_secondary(D, slot, nsec++, t, Tm, t.dx, t.dy, t.dz, P_ELECTRON);
-    else edep += Tm;
-    stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
-    finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+    do_pair(D, slot, k_iter, a, b);
   }
 }
 
 // S8 annihilation at rest: two photons of m_e, back to back, isotropic
+__device__ __forceinline__ void do_annihilation(const DeviceState& D, uint32_t slot, uint32_t k_iter, const RecA& a, const RecB& b) {
+  Track t = unpack(a, b);
+  double xi0, xi1;
+  draw_pair(D.P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+  const double cost = 2.0 * xi0 - 1.0;
+  const double sint = sqrt(1.0 - cost * cost);
+  double sp, cp;
+  sincospi(2.0 * xi1, &sp, &cp);
+  const double ux = sint * cp, uy = sint * sp, uz = cost;
+  stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
+  stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
+  finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
+}
 __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
   CEL_FOR_RANGE(R_ANNIH) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_ANNIH) continue;
     const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     if (meta_action(b.meta) != A_ANNIH) continue;
-    Track t = unpack(load_a(D.stA + slot), b);
-    double xi0, xi1;
-    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
-    const double cost = 2.0 * xi0 - 1.0;
-    const double sint = sqrt(1.0 - cost * cost);
-    double sp, cp;
-    sincospi(2.0 * xi1, &sp, &cp);
-    const double ux = sint * cp, uy = sint * sp, uz = cost;
-    stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
-    stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
-    finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
+    do_annihilation(D, slot, k_iter, a, b);
   }
 }
 
@@ -259,23 +273,29 @@ __device__ __forceinline__ int move_photon(const DeviceState& D, uint32_t slot, 
   return A_MOVE_G;
 }
 
+// act = COMPTON: interact, then (if the photon survives) move; act = MOVE_G: move
+template <int GEOM>
+__device__ __forceinline__ void do_photon(const DeviceState& D, uint32_t slot, uint32_t k_iter, const RecA& a, const RecB& b, int act) {
+  Track t = unpack(a, b);
+  const int vol0 = t.vol;
+  double edep = 0.0, eesc = 0.0;
+  int nsec = 0;
+  int action = A_VACANT;
+  bool alive = true;
+  if (act == A_COMPTON) alive = compton(D, slot, k_iter, t, edep, nsec);
+  if (alive) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
+  finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+}
 template <int GEOM>
 __global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
   CEL_FOR_RANGE(R_PHOTON) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_COMPTON && ak != A_MOVE_G) continue; }
     const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     const int act = meta_action(b.meta);
     if (act != A_COMPTON && act != A_MOVE_G) continue;
-    Track t = unpack(load_a(D.stA + slot), b);
-    const int vol0 = t.vol;
-    double edep = 0.0, eesc = 0.0;
-    int nsec = 0;
-    int action = A_VACANT;
-    bool alive = true;
-    if (act == A_COMPTON) alive = compton(D, slot, k_iter, t, edep, nsec);
-    if (alive) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
-    finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+    do_photon<GEOM>(D, slot, k_iter, a, b, act);
   }
 }
 
@@ -412,30 +432,37 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
   return (interaction_wins && complete) ? A_BREMS : A_MOVE_C;
 }
 
+// act = BREMS: interact, then (unless the track stopped) move; act = MOVE_C: move
+template <bool FIELD, int GEOM>
+__device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, uint32_t k_iter, const RecA& a, const RecB& b, int act) {
+  const Params& P = D.P;
+  Track t = unpack(a, b);
+  const int vol0 = t.vol;
+  double edep = 0.0, eesc = 0.0;
+  int nsec = 0;
+  int action = A_MOVE_C;
+  if (act == A_BREMS) {  // S8: k log-uniform on [k_c, T]; photon collinear
+    double xi0, xi1;
+    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+    const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
+    stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
+    const double T1 = t.a.energy - kph;
+    if (T1 < P.cut) { edep += T1; t.a.energy = 0.0; action = stop_charged(P, t.ptype, edep); }
+    else t.a.energy = T1;
+  }
+  if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
+  finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+}
 template <bool FIELD, int GEOM>
 __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }
     const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     const int act = meta_action(b.meta);
     if (act != A_MOVE_C && act != A_BREMS) continue;
-    Track t = unpack(load_a(D.stA + slot), b);
-    const int vol0 = t.vol;
-    double edep = 0.0, eesc = 0.0;
-    int nsec = 0;
-    int action = A_MOVE_C;
-    if (act == A_BREMS) {  // S8: k log-uniform on [k_c, T]; photon collinear
-      double xi0, xi1;
-      draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
-      const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
-      stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
-      const double T1 = t.a.energy - kph;
-      if (T1 < P.cut) { edep += T1; t.a.energy = 0.0; action = stop_charged(P, t.ptype, edep); }
-      else t.a.energy = T1;
-    }
-    if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
-    finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+    do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
   }
 }
 

@@ -14,11 +14,27 @@ M_E = 0.51099895
 TOL = 1e-12
 
 
-@pytest.fixture(scope="module")
-def binding():
+class _ExecutionForm:
+    """the binding module, with every context switched to one execution form of the iteration: the persistent
+    cooperative kernel (cel_persistent.cuh, the default) or the kernel-per-action CUDA graph"""
+
+    def __init__(self, b, persistent):
+        self._b, self._persistent = b, persistent
+
+    def __getattr__(self, name):
+        return getattr(self._b, name)
+
+    def from_workload(self, *a, **k):
+        ctx = self._b.from_workload(*a, **k)
+        ctx.set_option("persistent", self._persistent)
+        return ctx
+
+
+@pytest.fixture(scope="module", params=["persistent", "kernels"])
+def binding(request):
     from paper_2503_17608_b200 import binding as b
     b.load_library()
-    return b
+    return _ExecutionForm(b, 1 if request.param == "persistent" else 0)
 
 
 def compare_states(g, o, where=""):
@@ -170,6 +186,19 @@ def test_graph_and_direct_launch_identical(binding):
     a, ca = run_gpu(binding, w, use_graph=1, batch=16)
     b, cb = run_gpu(binding, w, use_graph=0, batch=3)
     assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb)
+
+
+def test_persistent_and_kernel_forms_identical(binding):
+    """the persistent cooperative kernel and the kernel-per-action graph are the same algorithm: tallies, per-iteration
+    action counts and counters agree bit-exactly in every sort mode (slab + field, and the cylinder geometry)"""
+    for w0 in (W.config3(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
+        for mode in (0, 1, 2):
+            w0.sort_mode = mode
+            a, ca = run_gpu(binding, w0, persistent=1, persist_batch=7)
+            b, cb = run_gpu(binding, w0, persistent=0)
+            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
+            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
+            assert a["kernel_launches"] < b["kernel_launches"]
 
 
 def three_sigma(gt, ot):
