@@ -198,8 +198,21 @@ __device__ __forceinline__ double lerp_node(double y0, double y1, double f) { re
 
 // Rinv(r): largest j <= 575 with R_j <= r, scanning down from j_hint (the cell of the pre-step energy; r <= R(T0))
 __device__ __forceinline__ double range_inverse(const Params& P, const double* __restrict__ R, double r, int j_hint) {
+  // gallop down from the hint (r is usually within a few cells of it: one step costs at most 20 % of the range),
+  // then bisect: a handful of loads for every lane instead of a per-lane linear scan. R is strictly increasing, so
+  // this is the same j as the plain downward scan.
   int j = j_hint;
-  while (j > 0 && __ldg(R + j) > r) --j;
+  if (__ldg(R + j) > r) {
+    int hi = j, step = 1;                      // invariant: R[hi] > r
+    int lo = hi - 1;
+    while (lo > 0 && __ldg(R + lo) > r) { hi = lo; step <<= 1; lo = hi - step; if (lo < 0) lo = 0; }
+    if (lo < 0) lo = 0;
+    while (hi - lo > 1) {                      // invariant: R[lo] <= r or lo == 0
+      const int mid = (lo + hi) >> 1;
+      if (__ldg(R + mid) > r) hi = mid; else lo = mid;
+    }
+    j = lo;
+  }
   const double Rj = __ldg(R + j), Rj1 = __ldg(R + j + 1);
   // T = exp(u_j + x) = E_j * exp(x), x = du (r - R_j)/(R_j+1 - R_j) in [0, du], du = ln(10)/64 = 0.036:
   // the degree-8 Taylor polynomial of exp is exact to 1e-17 there

@@ -204,13 +204,13 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
     // warp totals: at most 128 per key, so the 8-bit fields cannot carry
     a_lo = __reduce_add_sync(0xffffffffu, a_lo); a_hi = __reduce_add_sync(0xffffffffu, a_hi);
     if (D.sort_mode == 2) s_lo = __reduce_add_sync(0xffffffffu, s_lo);
-    if ((threadIdx.x & 31) == 0) {
-#pragma unroll
-      for (int a = 0; a < 4; ++a) {
-        const uint32_t lo = (a_lo >> (8 * a)) & 0xff, hi = (a_hi >> (8 * a)) & 0xff;
-        if (lo) atomicAdd(&sm.act[a], lo);
-        if (hi) atomicAdd(&sm.act[a + 4], hi);
-        if (D.sort_mode == 2) { const uint32_t h = (s_lo >> (8 * a)) & 0xff; if (h) atomicAdd(&sm.hist[a], h); }
+    {  // lanes 0-7 add the warp's count of key `lane`
+      const uint32_t lane = threadIdx.x & 31;
+      if (lane < 8) {
+        const uint32_t sh = 8 * (lane & 3);
+        const uint32_t a = ((lane < 4 ? a_lo : a_hi) >> sh) & 0xff;
+        if (a) atomicAdd(&sm.act[lane], a);
+        if (D.sort_mode == 2 && lane < 4) { const uint32_t h = (s_lo >> sh) & 0xff; if (h) atomicAdd(&sm.hist[lane], h); }
       }
     }
   }
@@ -289,8 +289,10 @@ __device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, ui
     if (c) {
 #pragma unroll
       for (int i = 0; i < kKeysPerThread; ++i) {
-        const uint32_t n = (nv >> (8 * i)) & 0xff;
-        for (uint32_t j = 0; j < n; ++j) sm.list[r++] = 2u * (base + i) + j;
+        const uint32_t n = (nv >> (8 * i)) & 0xff;     // 0, 1 or 2
+        if (n >= 1) sm.list[r] = 2u * (base + i);
+        if (n >= 2) sm.list[r + 1] = 2u * (base + i) + 1u;
+        r += n;
       }
       *reinterpret_cast<uint32_t*>(D.nsec + base) = 0u;   // consumed
     }
