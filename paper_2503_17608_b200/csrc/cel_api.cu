@@ -547,12 +547,14 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   if (c->d_tally) { CEL_CUDA(c, cudaFreeAsync(c->d_tally, s)); c->d_tally = nullptr; }
   const uint64_t tiles = D.n_tiles;
   const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
-  const uint64_t scratch_bytes = align_up(o_hist + tiles * 32, 256);
+  const uint64_t o_phist = align_up(o_hist + tiles * 32, 256);
+  const uint64_t scratch_bytes = align_up(o_phist + tiles * 32, 256);
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
   const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
   CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));
   D.tile_vac = (uint32_t*)((char*)c->scratch + o_vac);
   D.tile_hist = (uint32_t*)((char*)c->scratch + o_hist);
+  D.tile_phist = (uint32_t*)((char*)c->scratch + o_phist);
   D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
   D.tally = (unsigned long long*)c->d_tally;
   D.n_events = n_events;

@@ -112,7 +112,6 @@ struct Control {
   int32_t error;
   uint32_t offsets[9];              // offsets of the sorted index array, per sort key
   uint32_t counts[8];               // action counts of this iteration (after P1)
-  uint32_t counts_acc[8];           // accumulators (zero between iterations)
   uint32_t rb[8], re[8];            // index range of each action kernel for this iteration (KernelRange)
   uint32_t ticket_fill, ticket_push;
   uint32_t n_logged;
@@ -144,7 +143,8 @@ struct DeviceState {
   // stream-ordered scratch (cudaMallocAsync, per transport call)
   uint32_t* tile_vac;     // [n_tiles] vacant slots per tile: += by the action kernels, -= by the fill
   uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
-  uint32_t* tile_hist;    // [n_tiles][8] per-tile sort-key histogram -> exclusive base per key after k_init_fill
+  uint32_t* tile_hist;    // [n_tiles][8] per-tile action histogram (-> exclusive base per key after k_init_fill, sort by action)
+  uint32_t* tile_phist;   // [n_tiles][8] per-tile particle histogram, 4 used (sort by particle)
 };
 
 // ---------------------------------------------------------------- programmatic dependent launch (sm_90+)

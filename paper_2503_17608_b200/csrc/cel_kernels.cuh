@@ -215,13 +215,52 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
     }
   }
 }
-// after fill_tile + __syncthreads: publish the tile's sort-key histogram and add its action counts to the iteration's
+// after fill_tile + __syncthreads: publish the tile's action histogram and (sort by particle) its sort-key histogram.
+// The iteration's action counts are the column sums of tile_hist (no same-address atomics from a thousand blocks).
 __device__ __forceinline__ void publish_tile_hist(const DeviceState& D, BookSmem& sm, uint32_t tile) {
   if (threadIdx.x < 8) {
-    const uint32_t a = sm.act[threadIdx.x];
-    D.tile_hist[tile * 8 + threadIdx.x] = (D.sort_mode == 2) ? sm.hist[threadIdx.x] : a;
-    if (a) atomicAdd(&D.ctl->counts_acc[threadIdx.x], a);
+    D.tile_hist[tile * 8 + threadIdx.x] = sm.act[threadIdx.x];
+    if (D.sort_mode == 2) D.tile_phist[tile * 8 + threadIdx.x] = threadIdx.x < 4 ? sm.hist[threadIdx.x] : 0u;
   }
+}
+// the rows the scatter takes its per-tile bases from: the action histogram (sort by action) or the particle histogram
+__device__ __forceinline__ uint32_t* sort_rows(const DeviceState& D) { return D.sort_mode == 2 ? D.tile_phist : D.tile_hist; }
+
+// in-place exclusive scan over the tiles of the 8 columns of rows[n_tiles][8] by one block, in one pass: thread t owns
+// the tiles [t0, t1); the column totals go to total[8] (shared). write_back = false only computes the totals.
+__device__ __forceinline__ void scan_tile_rows(uint32_t* rows, uint32_t t0, uint32_t t1, bool write_back,
+                                               uint32_t (*warp_tot)[8] /* shared [8][8] */, uint32_t* total /* shared 8 */) {
+  uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (uint32_t t = t0; t < t1; ++t) {
+    const uint4 a = *reinterpret_cast<const uint4*>(rows + t * 8), b = *reinterpret_cast<const uint4*>(rows + t * 8 + 4);
+    acc[0] += a.x; acc[1] += a.y; acc[2] += a.z; acc[3] += a.w; acc[4] += b.x; acc[5] += b.y; acc[6] += b.z; acc[7] += b.w;
+  }
+  uint32_t ex[8];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const uint32_t incl = warp_incl_scan(acc[k]);
+    ex[k] = incl - acc[k];
+    if (lane == 31) warp_tot[warp][k] = incl;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    uint32_t before = 0, all = 0;
+#pragma unroll
+    for (int w = 0; w < kTileThreads / 32; ++w) { const uint32_t v = warp_tot[w][k]; all += v; if (w < warp) before += v; }
+    ex[k] += before;
+    if (threadIdx.x == 0) total[k] = all;
+  }
+  if (write_back) {
+    for (uint32_t t = t0; t < t1; ++t) {
+      uint4* pa = reinterpret_cast<uint4*>(rows + t * 8); uint4* pb = reinterpret_cast<uint4*>(rows + t * 8 + 4);
+      const uint4 a = *pa, b = *pb;
+      *pa = make_uint4(ex[0], ex[1], ex[2], ex[3]); *pb = make_uint4(ex[4], ex[5], ex[6], ex[7]);
+      ex[0] += a.x; ex[1] += a.y; ex[2] += a.z; ex[3] += a.w; ex[4] += b.x; ex[5] += b.y; ex[6] += b.z; ex[7] += b.w;
+    }
+  }
+  __syncthreads();
 }
 // vacancies of a tile that the fill of this iteration takes: min(v, max(0, n_take - (vacancies before the tile)))
 __device__ __forceinline__ uint32_t filled_in_tile(uint32_t v, uint32_t prefix, uint32_t n_take) {
@@ -328,11 +367,11 @@ __device__ __forceinline__ void set_ranges(const DeviceState& D, const uint32_t*
   }
 }
 // end-of-P1 bookkeeping of the control block by one thread (S11): counts, offsets, ranges, I, alive, log
-__device__ __forceinline__ void update_control_after_fill(const DeviceState& D, const uint32_t* key_total, int n_keys,
-                                                          unsigned long long I, uint32_t V, uint32_t n_take) {
+__device__ __forceinline__ void update_control_after_fill(const DeviceState& D, const uint32_t* act_total, const uint32_t* key_total,
+                                                          int n_keys, unsigned long long I, uint32_t V, uint32_t n_take) {
   Control* ctl = D.ctl;
   uint32_t cnt[8];
-  for (int a = 0; a < 8; ++a) { cnt[a] = ctl->counts_acc[a]; ctl->counts[a] = cnt[a]; ctl->counts_acc[a] = 0; }
+  for (int a = 0; a < 8; ++a) { cnt[a] = act_total[a]; ctl->counts[a] = cnt[a]; }
   const uint32_t N = D.N;
   uint32_t off[9];
   off[0] = 0;
@@ -392,42 +431,14 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
       ex += v[i];
     }
   }
-  // per-key exclusive scan of tile_hist over the tiles, all keys in one pass
-  __shared__ uint32_t key_total[8];
+  // column sums of the action histogram = the iteration's action counts; exclusive scan over the tiles of the rows the
+  // scatter uses (in place)
+  __shared__ uint32_t act_total[8], key_total[8];
   __shared__ uint32_t warp_tot[kTileThreads / 32][8];
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
-  if (n_keys) {
-    uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    for (uint32_t t = t0; t < t1; ++t) {
-      const uint4 a = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8), b = *reinterpret_cast<const uint4*>(D.tile_hist + t * 8 + 4);
-      acc[0] += a.x; acc[1] += a.y; acc[2] += a.z; acc[3] += a.w; acc[4] += b.x; acc[5] += b.y; acc[6] += b.z; acc[7] += b.w;
-    }
-    uint32_t ex[8];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      const uint32_t incl = warp_incl_scan(acc[k]);
-      ex[k] = incl - acc[k];
-      if (lane == 31) warp_tot[warp][k] = incl;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      uint32_t before = 0, all = 0;
-#pragma unroll
-      for (int w = 0; w < kTileThreads / 32; ++w) { const uint32_t v = warp_tot[w][k]; all += v; if (w < warp) before += v; }
-      ex[k] += before;
-      if (threadIdx.x == 0) key_total[k] = all;
-    }
-    for (uint32_t t = t0; t < t1; ++t) {
-      uint4* pa = reinterpret_cast<uint4*>(D.tile_hist + t * 8); uint4* pb = reinterpret_cast<uint4*>(D.tile_hist + t * 8 + 4);
-      const uint4 a = *pa, b = *pb;
-      *pa = make_uint4(ex[0], ex[1], ex[2], ex[3]); *pb = make_uint4(ex[4], ex[5], ex[6], ex[7]);
-      ex[0] += a.x; ex[1] += a.y; ex[2] += a.z; ex[3] += a.w; ex[4] += b.x; ex[5] += b.y; ex[6] += b.z; ex[7] += b.w;
-    }
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) update_control_after_fill(D, key_total, n_keys, I, V, n_take);
+  scan_tile_rows(D.tile_hist, t0, t1, D.sort_mode == 1, warp_tot, act_total);
+  if (D.sort_mode == 2) scan_tile_rows(D.tile_phist, t0, t1, true, warp_tot, key_total);
+  if (threadIdx.x == 0) update_control_after_fill(D, act_total, D.sort_mode == 2 ? key_total : act_total, n_keys, I, V, n_take);
 }
 
 __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
@@ -436,7 +447,7 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   const Control* ctl = D.ctl;
   if (ctl->finished) return;
   const uint32_t tile = blockIdx.x;
-  if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + D.tile_hist[tile * 8 + threadIdx.x];
+  if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + sort_rows(D)[tile * 8 + threadIdx.x];
   __syncthreads();
   scatter_tile(D, sm, tile, D.tile_vac[tile]);
 }

@@ -116,7 +116,7 @@ constexpr int kMaxTilesPerBlock = 16;   // the host falls back to the kernel-per
 template <bool FIELD, int GEOM>
 __global__ void __launch_bounds__(kTileThreads, FIELD ? 2 : 3) k_persistent(DeviceState D, uint32_t max_iters) {
   __shared__ BookSmem sm;
-  __shared__ uint32_t key_total[8];
+  __shared__ uint32_t key_total[8], act_total[8];
   __shared__ uint32_t off_s[9];
   __shared__ uint32_t tv_s[kMaxTilesPerBlock];   // tile_vac of the own tiles as read in P1 (before any action kernel adds)
   Control* ctl = D.ctl;
@@ -159,15 +159,23 @@ __global__ void __launch_bounds__(kTileThreads, FIELD ? 2 : 3) k_persistent(Devi
     }
     grid_barrier(&ctl->barrier, epoch);
     // ------------------------------------------------------------ P2: offsets, tile_vac -= filled, scatter (S2)
+    // action counts = column sums of the action histogram (the leader logs them); per-key bases from the rows the
+    // scatter sorts by. sm.base = (tiles before tile0)[key] of those rows.
+    if (D.sort_mode == 2) {
+      if (blockIdx.x == 0) block_prefix_total8(D.tile_hist, D.n_tiles, tile0, sm, act_total);
+      block_prefix_total8(D.tile_phist, D.n_tiles, tile0, sm, key_total);
+    } else if (D.sort_mode == 1 || blockIdx.x == 0) {
+      block_prefix_total8(D.tile_hist, D.n_tiles, tile0, sm, key_total);
+      if (threadIdx.x < 8) act_total[threadIdx.x] = key_total[threadIdx.x];
+    }
     if (n_keys) {
-      block_prefix_total8(D.tile_hist, D.n_tiles, tile0, sm, key_total);   // sm.base = (tiles before tile0)[key]
       if (threadIdx.x == 0) {
         off_s[0] = 0;
         for (int k = 0; k < 8; ++k) off_s[k + 1] = (k < n_keys) ? off_s[k] + key_total[k] : off_s[k];
       }
-      __syncthreads();
     }
-    if (leader) update_control_after_fill(D, key_total, n_keys, I, V, n_take);
+    __syncthreads();
+    if (leader) update_control_after_fill(D, act_total, key_total, n_keys, I, V, n_take);
     {
       uint32_t pv = prefix_v;
       uint32_t run = (threadIdx.x < 8 && n_keys) ? sm.base[threadIdx.x] : 0;   // thread k carries key k's running base
@@ -177,7 +185,7 @@ __global__ void __launch_bounds__(kTileThreads, FIELD ? 2 : 3) k_persistent(Devi
         pv += tv;
         if (n_keys) {
           __syncthreads();
-          if (threadIdx.x < 8) { sm.base[threadIdx.x] = off_s[threadIdx.x] + run; run += D.tile_hist[tile * 8 + threadIdx.x]; }
+          if (threadIdx.x < 8) { sm.base[threadIdx.x] = off_s[threadIdx.x] + run; run += sort_rows(D)[tile * 8 + threadIdx.x]; }
           __syncthreads();
           scatter_tile(D, sm, tile, tv - filled);
         }
