@@ -136,8 +136,17 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * profile: 1 = launch the kernels directly, one after the other, with a CUDA event after each one and synchronise once
  * per batch, so that cel_kernel_times can report per-kernel device time (a measurement mode: results are identical,
  * the run is slower). concurrent: 1 (default) = the independent action kernels of an iteration run as parallel
- * branches of the iteration graph; 0 = one after the other. */
+ * branches of the iteration graph; 0 = one after the other. pdl: programmatic dependent launch along the main
+ * chain (default 1). persistent: the cooperative one-kernel form (default 0). trace: see cel_trace. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
+
+/* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a
+ * transport makes every kernel of the first n iterations stamp the GPU's global nanosecond timer when its first block
+ * starts and when its last warp ends (two integer atomics per warp: a measurement mode, results are identical).
+ * cel_trace copies the stamps to the HOST array host_out[n][CEL_KERNEL_COUNT][2] = {start_ns, end_ns} (caller-owned;
+ * may be NULL to query n) and sets *n_iters = n; a kernel that did not run in an iteration (or an iteration that was
+ * never reached) keeps {UINT64_MAX, 0}. Synchronises the stream. Errors: INVALID_ARG, NOT_RUN, CUDA. */
+int cel_trace(cel_ctx*, uint64_t* host_out, uint64_t* n_iters);
 
 /* ---- debug / parity surface (synchronous, not timed) ---- */
 int cel_debug_begin(cel_ctx*, const cel_primary* primaries, uint64_t n, uint32_t n_events); /* load only */

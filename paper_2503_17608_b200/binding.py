@@ -20,7 +20,7 @@ EXPORTS = ["cel_create", "cel_set_stream", "cel_workspace_bytes", "cel_set_works
            "cel_transport_device", "cel_tallies", "cel_destroy", "cel_strerror", "cel_last_cuda_error", "cel_set_option",
            "cel_debug_begin", "cel_debug_step", "cel_debug_read_state", "cel_debug_read_indices",
            "cel_debug_n_initializers", "cel_debug_read_initializers", "cel_debug_n_counts", "cel_debug_read_counts",
-           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times"]
+           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace"]
 
 
 class cel_material(C.Structure):
@@ -93,6 +93,7 @@ def load_library():
     L.cel_kernel_name.restype = C.c_char_p
     L.cel_kernel_name.argtypes = [C.c_int]
     L.cel_kernel_times.argtypes = [vp, vp, vp]
+    L.cel_trace.argtypes = [vp, vp, vp]
     _lib = L
     return L
 
@@ -195,6 +196,16 @@ class Context:
         ms = np.zeros(n); cnt = np.zeros(n, np.uint64)
         self._check(L.cel_kernel_times(self.h, _p(ms), _p(cnt)), "cel_kernel_times")
         return {L.cel_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n)}
+
+    def trace(self):
+        """(kernel names, stamps[n_iters][n_kernels][2] uint64 ns) of the last transport run with option trace=n"""
+        L = load_library()
+        n = C.c_uint64(0)
+        self._check(L.cel_trace(self.h, None, C.byref(n)), "cel_trace")
+        out = np.zeros((n.value, L.cel_kernel_count(), 2), np.uint64)
+        if n.value:
+            self._check(L.cel_trace(self.h, _p(out), C.byref(n)), "cel_trace")
+        return [L.cel_kernel_name(i).decode() for i in range(L.cel_kernel_count())], out
 
     # ---- debug / parity surface
     def begin(self, primaries, n_events):

@@ -16,6 +16,7 @@ using namespace cel;
 
 static_assert(sizeof(cel_primary) == 64 && sizeof(PrimaryRec) == 64, "cel_primary layout");
 static_assert(sizeof(cel_track) == 80 && sizeof(TrackRec) == 80, "cel_track layout");
+static_assert((int)K_COUNT == (int)CEL_KERNEL_COUNT && (int)K_PUSH == (int)CEL_K_PUSH && (int)K_CHARGED == (int)CEL_K_CHARGED, "kernel ids");
 static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32, "record layout");
 static_assert(sizeof(DeviceState) < 3500, "DeviceState must fit in kernel parameter space");
 
@@ -57,6 +58,8 @@ struct cel_ctx {
   uint64_t* h_tally = nullptr; size_t h_tally_bytes = 0;   // pinned
   void* h_prim = nullptr; size_t h_prim_bytes = 0;         // pinned staging of primaries
   cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
+  int trace_iters = 0; void* d_trace = nullptr;   // option "trace": device-side timeline of the first trace_iters iterations
+  DeviceState graph_D{}; int graph_cfg[3] = {-1, -1, -1};   // what the captured graph has baked in (arguments, options)
   int use_graph = 1; int batch = 16; int64_t max_iterations = 1ll << 22;
   int persistent = 0; int persist_batch = 64;   // one cooperative kernel runs up to persist_batch iterations
   int persist_grid = 0;                         // co-resident blocks of k_persistent (0 = not available)
@@ -357,6 +360,7 @@ extern "C" void cel_destroy(cel_ctx* c) {
   if (c->scratch) cudaFree(c->scratch);
   if (c->d_tally) cudaFree(c->d_tally);
   if (c->d_prim) cudaFree(c->d_prim);
+  if (c->d_trace) cudaFree(c->d_trace);
   if (c->own_workspace && c->workspace) cudaFree(c->workspace);
   if (c->d_params_blob) cudaFree(c->d_params_blob);
   if (c->h_status) cudaFreeHost(c->h_status);
@@ -394,6 +398,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "concurrent")) c->concurrent = v ? 1 : 0;
   else if (!std::strcmp(name, "persistent")) c->persistent = v ? 1 : 0;
   else if (!std::strcmp(name, "pdl")) c->pdl = v ? 1 : 0;
+  else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
   else if (!std::strcmp(name, "persist_batch")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->persist_batch = (int)v; }
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
@@ -558,6 +563,17 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
   D.tally = (unsigned long long*)c->d_tally;
   D.n_events = n_events;
+  if (c->d_trace) { CEL_CUDA(c, cudaFreeAsync(c->d_trace, s)); c->d_trace = nullptr; }
+  D.trace = nullptr; D.trace_iters = 0;
+  if (c->trace_iters > 0) {   // [iters][K_COUNT][2]: starts = ~0 (atomicMin), ends = 0 (atomicMax)
+    const size_t n = (size_t)c->trace_iters * K_COUNT * 2;
+    CEL_CUDA(c, cudaMallocAsync(&c->d_trace, n * 8, s));
+    std::vector<unsigned long long> init(n);
+    for (size_t i = 0; i < n; ++i) init[i] = (i & 1) ? 0ull : ~0ull;
+    CEL_CUDA(c, cudaMemcpyAsync(c->d_trace, init.data(), n * 8, cudaMemcpyHostToDevice, s));
+    CEL_CUDA(c, cudaStreamSynchronize(s));   // `init` is pageable host memory (measurement mode only)
+    D.trace = (unsigned long long*)c->d_trace; D.trace_iters = (uint32_t)c->trace_iters;
+  }
   CEL_CUDA(c, cudaMemsetAsync(c->scratch, 0, scratch_bytes, s));
   CEL_CUDA(c, cudaMemsetAsync(c->d_tally, 0, tally_bytes > 0 ? tally_bytes : 8, s));
   CEL_CUDA(c, cudaMemsetAsync(D.ctl, 0, sizeof(Control), s));
@@ -571,8 +587,15 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
     c->h_tally_bytes = tally_bytes;
   }
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
-  if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
-  if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+  // (the stream-ordered pool hands the same scratch back run after run, so the graph of the last run is normally
+  // still valid: it is kept when every baked-in argument and option is unchanged)
+  const int cfg[3] = {c->batch, c->concurrent, c->pdl};
+  const bool graph_valid = c->graph_exec && std::memcmp(&c->graph_D, &D, sizeof(DeviceState)) == 0 &&
+                           std::memcmp(c->graph_cfg, cfg, sizeof(cfg)) == 0;
+  if (!graph_valid) {
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+  }
   for (int i = 0; i < CEL_KERNEL_COUNT; ++i) { c->kernel_ms[i] = 0.0; c->kernel_launches[i] = 0; }
   if (c->profile) {
     const size_t need = (size_t)c->batch * (kMaxKernelsPerIteration + 1);
@@ -582,12 +605,14 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
       c->prof_ev.push_back(e);
     }
   }
-  if (c->use_graph && !c->profile && !use_persistent(c)) {
+  if (c->use_graph && !c->profile && !use_persistent(c) && !graph_valid) {
     // one graph = one batch of iterations: a single cudaGraphLaunch per status poll keeps the host far ahead of the device
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     for (int b = 0; b < c->batch; ++b) c->kernels_per_iteration = enqueue_iteration(c);
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
     CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
+    std::memcpy(&c->graph_D, &D, sizeof(DeviceState));
+    std::memcpy(c->graph_cfg, cfg, sizeof(cfg));
   }
   c->launches = 1; c->run_error = 0; c->ran = true;   // k_reset_state
   std::memset(&c->last, 0, sizeof(Control));
@@ -643,7 +668,7 @@ int run_loop(cel_ctx* c) {
       int prc = launch_persistent(c, (uint32_t)c->persist_batch);
       if (prc != CEL_OK) return prc;
       enqueued += c->persist_batch - c->batch;
-    } else if (c->graph_exec) {
+    } else if (c->graph_exec && c->use_graph && !c->profile) {
       CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s));
       c->launches += (uint64_t)c->kernels_per_iteration * c->batch;
     } else {
@@ -712,6 +737,16 @@ extern "C" int cel_tallies(cel_ctx* c, cel_tally_view* out) {
   out->kernel_launches = c->launches;
   if (c->last.error != 0) return c->last.error;
   return c->run_error;
+}
+
+extern "C" int cel_trace(cel_ctx* c, uint64_t* host_out, uint64_t* n_iters) {
+  if (!c || !n_iters) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  const uint64_t n = c->d_trace ? (uint64_t)c->D.trace_iters : 0;
+  *n_iters = n;
+  if (host_out && n) CEL_CUDA(c, cudaMemcpy(host_out, c->d_trace, n * K_COUNT * 2 * 8, cudaMemcpyDeviceToHost));
+  return CEL_OK;
 }
 
 extern "C" int cel_kernel_count(void) { return CEL_KERNEL_COUNT; }

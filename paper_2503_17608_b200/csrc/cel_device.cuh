@@ -145,6 +145,48 @@ struct DeviceState {
   uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
   uint32_t* tile_hist;    // [n_tiles][8] per-tile action histogram (-> exclusive base per key after k_init_fill, sort by action)
   uint32_t* tile_phist;   // [n_tiles][8] per-tile particle histogram, 4 used (sort by particle)
+  // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
+  // in / last warp out of every kernel of every iteration; nullptr = off
+  unsigned long long* trace;
+  uint32_t trace_iters;
+};
+
+// kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
+enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_COUNT };
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+  return t;
+}
+// scope object of a kernel body: stamps the kernel's [start, end] of iteration `iter` when tracing is on. One global
+// atomic per block and stamp at most: the block's warps count themselves out in shared memory and the last one stamps
+// the end; a plain read first skips the atomic when the stamp cannot change.
+struct TraceScope {
+  unsigned long long* p;
+  unsigned int* done;
+  __device__ __forceinline__ TraceScope(const DeviceState& D, uint32_t iter, int kid) {
+    __shared__ unsigned int s_done;
+    done = &s_done;
+    p = (D.trace != nullptr && iter < D.trace_iters) ? D.trace + ((size_t)iter * K_COUNT + kid) * 2 : nullptr;
+    if (p != nullptr) {   // block-uniform
+      if (threadIdx.x == 0) {
+        s_done = 0;
+        const unsigned long long now = globaltimer_ns();
+        if (now < *reinterpret_cast<volatile unsigned long long*>(p)) atomicMin(p, now);
+      }
+      __syncthreads();
+    }
+  }
+  __device__ __forceinline__ ~TraceScope() {
+    if (p != nullptr && (threadIdx.x & 31) == 0) {
+      const unsigned int warps = (blockDim.x + 31) >> 5;
+      if (atomicAdd(done, 1u) == warps - 1) {
+        const unsigned long long now = globaltimer_ns();
+        if (now > *reinterpret_cast<volatile unsigned long long*>(p + 1)) atomicMax(p + 1, now);
+      }
+    }
+  }
 };
 
 // ---------------------------------------------------------------- programmatic dependent launch (sm_90+)

@@ -405,6 +405,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
+  const TraceScope trace(D, ctl->iter, K_INIT_FILL);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
@@ -446,6 +447,7 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
   if (ctl->finished) return;
+  const TraceScope trace(D, ctl->iter, K_SCATTER);
   const uint32_t tile = blockIdx.x;
   if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + sort_rows(D)[tile * 8 + threadIdx.x];
   __syncthreads();
@@ -457,6 +459,7 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
+  const TraceScope trace(D, ctl->iter, K_PUSH);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
   uint32_t prefix, S;

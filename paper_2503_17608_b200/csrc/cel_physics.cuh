@@ -111,12 +111,13 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 
 // ================================================================ P3i: pure interactions (the slot is vacated)
 // Loop over the kernel's index range with a grid-stride loop; `slot` is the gathered slot index.
-#define CEL_FOR_RANGE(RANGE_ID)                                                                             \
+#define CEL_FOR_RANGE(RANGE_ID, KERNEL_ID)                                                                  \
   pdl_prologue();                                                                                           \
   const Control* ctl = D.ctl;                                                                               \
   if (ctl->finished) return;                                                                                \
   const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
   const uint32_t k_iter = ctl->iter;                                                                        \
+  const TraceScope trace(D, k_iter, KERNEL_ID);                                                             \
   const Params& P = D.P;                                                                                    \
   (void)k_iter; (void)P;                                                                                    \
   for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x)
@@ -133,7 +134,7 @@ __device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t 
   finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
 }
 __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
-  CEL_FOR_RANGE(R_PE) {
+  CEL_FOR_RANGE(R_PE, K_PE) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PE) continue;
     const RecB b = load_b(D.stB + slot);
@@ -160,7 +161,7 @@ __device__ __forceinline__ void do_pair(const DeviceState& D, uint32_t slot, uin
   finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
 }
 __global__ void __launch_bounds__(kBlock) k_pair(DeviceState D) {
-  CEL_FOR_RANGE(R_PAIR) {
+  CEL_FOR_RANGE(R_PAIR, K_PAIR) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_PAIR) continue;
     const RecB b = load_b(D.stB + slot);
@@ -185,7 +186,7 @@ __device__ __forceinline__ void do_annihilation(const DeviceState& D, uint32_t s
   finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
 }
 __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
-  CEL_FOR_RANGE(R_ANNIH) {
+  CEL_FOR_RANGE(R_ANNIH, K_ANNIH) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1 && (D.akey[slot] & 0xf) != A_ANNIH) continue;
     const RecB b = load_b(D.stB + slot);
@@ -288,7 +289,7 @@ __device__ __forceinline__ void do_photon(const DeviceState& D, uint32_t slot, u
 }
 template <int GEOM>
 __global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
-  CEL_FOR_RANGE(R_PHOTON) {
+  CEL_FOR_RANGE(R_PHOTON, K_PHOTON) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_COMPTON && ak != A_MOVE_G) continue; }
     const RecB b = load_b(D.stB + slot);
@@ -455,7 +456,7 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
 }
 template <bool FIELD, int GEOM>
 __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
-  CEL_FOR_RANGE(R_CHARGED) {
+  CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }
     const RecB b = load_b(D.stB + slot);
