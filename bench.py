@@ -175,7 +175,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     rw = 2 * STATE_BYTES + idx          # gather + write back one slot through the index
     n = float(n_slots)
     sec = float(n_secondaries)
-    return {
+    out = {
         "init_fill": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES,   # key bytes + (read init, write slot)
         "scatter": it * n * (1 + INDEX_BYTES),
         "annihilation": c[6] * (rw + 2 * STATE_BYTES),
@@ -185,6 +185,9 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
         "charged": (c[4] + c[5]) * rw + c[5] * STATE_BYTES,                  # bremsstrahlung stages one photon
         "push": sec * (1 + 2 * STATE_BYTES),                                 # nsec byte + (read staging, write stack)
     }
+    # sorted by action the five action kernels are one launch (k_actions): the same bytes, summed
+    out["actions"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair", "photon", "charged"))
+    return out
 
 
 def measured_peaks():
@@ -196,17 +199,17 @@ def measured_peaks():
 
 
 def load_profile_traffic(kernel):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full summary
-    (profiles/traffic.txt: lines `kernel_name bytes_per_launch`), or None"""
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, iteration captured) from the committed
+    ncu --set full summary (profiles/traffic.txt: lines `kernel_name bytes_per_launch iteration`), or (None, None)"""
     path = os.path.join(ROOT, "profiles", "traffic.txt")
     if not os.path.exists(path):
-        return None
+        return None, None
     with open(path) as f:
         for line in f:
             parts = line.split()
             if len(parts) >= 2 and not line.startswith("#") and parts[0] == kernel:
-                return float(parts[1])
-    return None
+                return float(parts[1]), (int(parts[2]) if len(parts) > 2 else None)
+    return None, None
 
 
 # ---------------------------------------------------------------- the CUDA arm
@@ -323,8 +326,13 @@ def run_cuda(args):
                          "alg_bytes": alg[name], "gbs": round(gbs, 2), "frac": round(gbs / peak, 4)}
     dominant = max(kernels, key=lambda k: kernels[k]["ms"])
     dk = kernels[dominant]
+    traffic, traffic_it = load_profile_traffic(dominant)
+    alg_at_it = None
+    if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "actions"):
+        alg_at_it = algorithmic_bytes(counts[traffic_it:traffic_it + 1], w.n_slots, w.sort_mode, 0, 0)[dominant]
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": dk["frac"], "traffic": load_profile_traffic(dominant), "peak_kind": peak_kind,
+                "frac": dk["frac"], "traffic": traffic, "traffic_iteration": traffic_it,
+                "alg_bytes_at_traffic_iteration": alg_at_it, "peak_kind": peak_kind,
                 "alg_bytes_per_launch": dk["alg_bytes"] / dk["launches"], "avg_launch_us": 1e3 * dk["ms"] / dk["launches"],
                 "share_of_step": dk["share"], "iterations": int(pview["iterations"]),
                 "how": "profile pass after the timed steps: same workload, CUDA events around every kernel launch"}

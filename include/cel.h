@@ -122,7 +122,7 @@ const char* cel_last_cuda_error(cel_ctx*);
  * P3i: ANNIH, PE, PAIR; P3i+P3m: PHOTON (Compton, then the photon move), CHARGED (bremsstrahlung, then the charged move
  * with energy loss and MSC); P4 (scoring) happens inside the action kernels; P5: PUSH. */
 enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
-       CEL_KERNEL_COUNT };
+       CEL_K_ACTIONS /* the five action kernels in one launch (sort by action, option fused) */, CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
 /* Per-kernel device time of the last transport run with option "profile" = 1 (per-kernel HBM
@@ -137,7 +137,9 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * per batch, so that cel_kernel_times can report per-kernel device time (a measurement mode: results are identical,
  * the run is slower). concurrent: 1 (default) = the independent action kernels of an iteration run as parallel
  * branches of the iteration graph; 0 = one after the other. pdl: programmatic dependent launch along the main
- * chain (default 1). persistent: the cooperative one-kernel form (default 0). trace: see cel_trace. */
+ * chain (default 1). persistent: the cooperative one-kernel form (default 0). fused: sorted by action, launch the
+ * five action kernels as one grid that walks the chunks of every action's range (default 0 = one launch per
+ * action on parallel graph branches; measured equal without a field, slower with one). trace: see cel_trace. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a
@@ -145,7 +147,8 @@ int cel_set_option(cel_ctx*, const char* name, int64_t value);
  * starts and when its last warp ends (two integer atomics per warp: a measurement mode, results are identical).
  * cel_trace copies the stamps to the HOST array host_out[n][CEL_KERNEL_COUNT][2] = {start_ns, end_ns} (caller-owned;
  * may be NULL to query n) and sets *n_iters = n; a kernel that did not run in an iteration (or an iteration that was
- * never reached) keeps {UINT64_MAX, 0}. Synchronises the stream. Errors: INVALID_ARG, NOT_RUN, CUDA. */
+ * never reached) keeps {UINT64_MAX, 0}. cel_set_option("trace_ends", 0) stamps the starts only (no atomics at the end
+ * of a kernel: the least perturbing form; end_ns stays 0). Synchronises the stream. Errors: INVALID_ARG, NOT_RUN, CUDA. */
 int cel_trace(cel_ctx*, uint64_t* host_out, uint64_t* n_iters);
 
 /* ---- debug / parity surface (synchronous, not timed) ---- */

@@ -149,10 +149,11 @@ struct DeviceState {
   // in / last warp out of every kernel of every iteration; nullptr = off
   unsigned long long* trace;
   uint32_t trace_iters;
+  uint32_t trace_ends;    // 0 = start stamps only (no end-of-kernel atomics: the least perturbing form)
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_COUNT };
+enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
@@ -161,29 +162,36 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
 }
 // scope object of a kernel body: stamps the kernel's [start, end] of iteration `iter` when tracing is on. One global
 // atomic per block and stamp at most: the block's warps count themselves out in shared memory and the last one stamps
-// the end; a plain read first skips the atomic when the stamp cannot change.
+// the end; a plain read first skips the atomic when the stamp cannot change. Holds no pointer (the stamp address is
+// recomputed from the kernel parameters). Every kernel is compiled twice, TRACE = false being an empty object, so that
+// the untraced path keeps its code and its register count.
+template <int KID, bool TRACE>
 struct TraceScope {
-  unsigned long long* p;
-  unsigned int* done;
-  __device__ __forceinline__ TraceScope(const DeviceState& D, uint32_t iter, int kid) {
-    __shared__ unsigned int s_done;
-    done = &s_done;
-    p = (D.trace != nullptr && iter < D.trace_iters) ? D.trace + ((size_t)iter * K_COUNT + kid) * 2 : nullptr;
-    if (p != nullptr) {   // block-uniform
+  __device__ __forceinline__ TraceScope(const DeviceState&, uint32_t) {}
+};
+template <int KID>
+struct TraceScope<KID, true> {
+  const DeviceState& D;
+  const uint32_t iter;
+  static __device__ __forceinline__ unsigned int* done_counter() { __shared__ unsigned int s_done; return &s_done; }
+  __device__ __forceinline__ unsigned long long* stamp() const { return D.trace + ((size_t)iter * K_COUNT + KID) * 2; }
+  __device__ __forceinline__ bool on() const { return D.trace != nullptr && iter < D.trace_iters; }
+  __device__ __forceinline__ TraceScope(const DeviceState& D_, uint32_t iter_) : D(D_), iter(iter_) {
+    if (on()) {   // block-uniform
       if (threadIdx.x == 0) {
-        s_done = 0;
+        *done_counter() = 0;
         const unsigned long long now = globaltimer_ns();
-        if (now < *reinterpret_cast<volatile unsigned long long*>(p)) atomicMin(p, now);
+        if (now < *reinterpret_cast<volatile unsigned long long*>(stamp())) atomicMin(stamp(), now);
       }
       __syncthreads();
     }
   }
   __device__ __forceinline__ ~TraceScope() {
-    if (p != nullptr && (threadIdx.x & 31) == 0) {
+    if (on() && D.trace_ends && (threadIdx.x & 31) == 0) {
       const unsigned int warps = (blockDim.x + 31) >> 5;
-      if (atomicAdd(done, 1u) == warps - 1) {
+      if (atomicAdd(done_counter(), 1u) == warps - 1) {
         const unsigned long long now = globaltimer_ns();
-        if (now > *reinterpret_cast<volatile unsigned long long*>(p + 1)) atomicMax(p + 1, now);
+        if (now > *reinterpret_cast<volatile unsigned long long*>(stamp() + 1)) atomicMax(stamp() + 1, now);
       }
     }
   }

@@ -400,12 +400,13 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
 // ================================================================ the bookkeeping kernels (one block per tile)
 // k_init_fill: P1 + the per-tile histograms; its last block turns the histograms into per-key bases (exclusive scan
 // over the tiles), takes the filled vacancies off tile_vac, and updates offsets, ranges, counters and the log.
+template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
-  const TraceScope trace(D, ctl->iter, K_INIT_FILL);
+  const TraceScope<K_INIT_FILL, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
@@ -442,24 +443,26 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   if (threadIdx.x == 0) update_control_after_fill(D, act_total, D.sort_mode == 2 ? key_total : act_total, n_keys, I, V, n_take);
 }
 
+template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   const Control* ctl = D.ctl;
   if (ctl->finished) return;
-  const TraceScope trace(D, ctl->iter, K_SCATTER);
+  const TraceScope<K_SCATTER, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
   if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + sort_rows(D)[tile * 8 + threadIdx.x];
   __syncthreads();
   scatter_tile(D, sm, tile, D.tile_vac[tile]);
 }
 
+template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
-  const TraceScope trace(D, ctl->iter, K_PUSH);
+  const TraceScope<K_PUSH, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
   uint32_t prefix, S;

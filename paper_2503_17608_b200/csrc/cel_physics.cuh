@@ -117,7 +117,7 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
   if (ctl->finished) return;                                                                                \
   const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
   const uint32_t k_iter = ctl->iter;                                                                        \
-  const TraceScope trace(D, k_iter, KERNEL_ID);                                                             \
+  const TraceScope<KERNEL_ID, TRACE> trace(D, k_iter);                                                      \
   const Params& P = D.P;                                                                                    \
   (void)k_iter; (void)P;                                                                                    \
   for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x)
@@ -133,6 +133,7 @@ __device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t 
   else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
   finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
 }
+template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
   CEL_FOR_RANGE(R_PE, K_PE) {
     const uint32_t slot = slot_of(D, tid);
@@ -160,6 +161,7 @@ __device__ __forceinline__ void do_pair(const DeviceState& D, uint32_t slot, uin
   stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
   finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
 }
+template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_pair(DeviceState D) {
   CEL_FOR_RANGE(R_PAIR, K_PAIR) {
     const uint32_t slot = slot_of(D, tid);
@@ -185,6 +187,7 @@ __device__ __forceinline__ void do_annihilation(const DeviceState& D, uint32_t s
   stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
   finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
 }
+template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
   CEL_FOR_RANGE(R_ANNIH, K_ANNIH) {
     const uint32_t slot = slot_of(D, tid);
@@ -287,7 +290,7 @@ __device__ __forceinline__ void do_photon(const DeviceState& D, uint32_t slot, u
   if (alive) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
   finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
 }
-template <int GEOM>
+template <int GEOM, bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_photon(DeviceState D) {
   CEL_FOR_RANGE(R_PHOTON, K_PHOTON) {
     const uint32_t slot = slot_of(D, tid);
@@ -454,7 +457,7 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
   if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
   finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
 }
-template <bool FIELD, int GEOM>
+template <bool FIELD, int GEOM, bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
@@ -464,6 +467,69 @@ __global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
     const int act = meta_action(b.meta);
     if (act != A_MOVE_C && act != A_BREMS) continue;
     do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
+  }
+}
+
+// ================================================================ all action kernels in ONE launch (sort by action)
+// Sorted by action, every action owns a contiguous range of the index array. Instead of one launch per
+// action, the ranges are cut into chunks of kBlock indices and ONE grid walks the chunks of all ranges, heaviest action
+// first (charged, photon, annihilation, photoelectric, pair): a block still runs exactly one action's code on one
+// contiguous piece of that action's range — no masks, no divergence between actions inside a block — but the
+// iteration loses four launches, the fork / join of the side streams, and the tail in which the small kernels queued
+// behind the blocks of the big ones (profiles/: timeline). Results are bit-identical to the kernel-per-action form.
+template <bool FIELD, int GEOM, bool TRACE>
+__global__ void __launch_bounds__(kBlock) k_actions(DeviceState D) {
+  pdl_prologue();
+  const Control* ctl = D.ctl;
+  if (ctl->finished) return;
+  const uint32_t k_iter = ctl->iter;
+  const TraceScope<K_ACTIONS, TRACE> trace(D, k_iter);
+  // chunk ranges, in launch order
+  const uint32_t b_ch = ctl->rb[R_CHARGED], e_ch = ctl->re[R_CHARGED];
+  const uint32_t b_ph = ctl->rb[R_PHOTON], e_ph = ctl->re[R_PHOTON];
+  const uint32_t b_an = ctl->rb[R_ANNIH], e_an = ctl->re[R_ANNIH];
+  const uint32_t b_pe = ctl->rb[R_PE], e_pe = ctl->re[R_PE];
+  const uint32_t b_pa = ctl->rb[R_PAIR], e_pa = ctl->re[R_PAIR];
+  const uint32_t n_ch = (e_ch - b_ch + kBlock - 1) / kBlock, n_ph = (e_ph - b_ph + kBlock - 1) / kBlock;
+  const uint32_t n_an = (e_an - b_an + kBlock - 1) / kBlock, n_pe = (e_pe - b_pe + kBlock - 1) / kBlock;
+  const uint32_t n_pa = (e_pa - b_pa + kBlock - 1) / kBlock;
+  const uint32_t c1 = n_ch, c2 = c1 + n_ph, c3 = c2 + n_an, c4 = c3 + n_pe, c5 = c4 + n_pa;
+  for (uint32_t v = blockIdx.x; v < c5; v += gridDim.x) {   // block-uniform: one action per block and chunk
+    if (v < c1) {
+      const uint32_t tid = b_ch + v * kBlock + threadIdx.x;
+      if (tid < e_ch) {
+        const uint32_t slot = D.indices[tid];
+        const RecB b = load_b(D.stB + slot);
+        const RecA a = load_a(D.stA + slot);
+        const int act = meta_action(b.meta);
+        if (act == A_MOVE_C || act == A_BREMS) do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
+      }
+    } else if (v < c2) {
+      const uint32_t tid = b_ph + (v - c1) * kBlock + threadIdx.x;
+      if (tid < e_ph) {
+        const uint32_t slot = D.indices[tid];
+        const RecB b = load_b(D.stB + slot);
+        const RecA a = load_a(D.stA + slot);
+        const int act = meta_action(b.meta);
+        if (act == A_COMPTON || act == A_MOVE_G) do_photon<GEOM>(D, slot, k_iter, a, b, act);
+      }
+    } else {
+      uint32_t tid, end; int want;
+      if (v < c3) { tid = b_an + (v - c2) * kBlock; end = e_an; want = A_ANNIH; }
+      else if (v < c4) { tid = b_pe + (v - c3) * kBlock; end = e_pe; want = A_PE; }
+      else { tid = b_pa + (v - c4) * kBlock; end = e_pa; want = A_PAIR; }
+      tid += threadIdx.x;
+      if (tid < end) {
+        const uint32_t slot = D.indices[tid];
+        const RecB b = load_b(D.stB + slot);
+        const RecA a = load_a(D.stA + slot);
+        if (meta_action(b.meta) == want) {
+          if (want == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
+          else if (want == A_PE) do_photoelectric(D, slot, a, b);
+          else do_pair(D, slot, k_iter, a, b);
+        }
+      }
+    }
   }
 }
 
