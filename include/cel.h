@@ -163,6 +163,10 @@ int cel_debug_read_counts(cel_ctx*, uint32_t* host_out /* [n][8] */);
 int cel_debug_table(cel_ctx*, int material, int which /* 0 C, 1 PE, 2 pair, 3 brems, 4 range */, double* out577);
 int cel_debug_uniforms(cel_ctx*, const uint32_t* slots, uint32_t n, uint32_t k, uint32_t phase, uint32_t j,
                        double* host_out);                     /* xi_j(seed, slot, k, phase) evaluated on the device */
+/* The path's own elementary functions evaluated on the device, for the accuracy tests:
+ * which = 0: sin x, 1: 1 - cos x for |x| <= 0.5 (the helix angle of one chord substep, S7.3: Taylor polynomials, no
+ * argument reduction, no cancellation). host_in / host_out: HOST arrays of n doubles, caller-owned. */
+int cel_debug_math(cel_ctx*, int which, const double* host_in, uint32_t n, double* host_out);
 
 #ifdef __cplusplus
 }

@@ -20,7 +20,7 @@ EXPORTS = ["cel_create", "cel_set_stream", "cel_workspace_bytes", "cel_set_works
            "cel_transport_device", "cel_tallies", "cel_destroy", "cel_strerror", "cel_last_cuda_error", "cel_set_option",
            "cel_debug_begin", "cel_debug_step", "cel_debug_read_state", "cel_debug_read_indices",
            "cel_debug_n_initializers", "cel_debug_read_initializers", "cel_debug_n_counts", "cel_debug_read_counts",
-           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace"]
+           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace", "cel_debug_math"]
 
 
 class cel_material(C.Structure):
@@ -250,6 +250,12 @@ class Context:
     def uniforms(self, slots, k, phase, j):
         s = np.ascontiguousarray(slots, dtype=np.uint32); out = np.zeros(len(s))
         self._check(load_library().cel_debug_uniforms(self.h, _p(s), len(s), k, phase, j, _p(out)), "cel_debug_uniforms")
+        return out
+
+    def debug_math(self, which, x):
+        """the path's small-angle sin (which=0) and 1 - cos (1) of the helix substep, evaluated on the device"""
+        a = np.ascontiguousarray(x, dtype=np.float64); out = np.zeros(len(a))
+        self._check(load_library().cel_debug_math(self.h, int(which), _p(a), len(a), _p(out)), "cel_debug_math")
         return out
 
 

@@ -907,3 +907,19 @@ extern "C" int cel_debug_uniforms(cel_ctx* c, const uint32_t* slots, uint32_t n,
   CEL_CUDA(c, cudaStreamSynchronize(c->stream));
   return CEL_OK;
 }
+
+extern "C" int cel_debug_math(cel_ctx* c, int which, const double* host_in, uint32_t n, double* host_out) {
+  if (!c || !host_in || !host_out || which < 0 || which > 1) return CEL_ERR_INVALID_ARG;
+  if (n == 0) return CEL_OK;
+  void* din = nullptr; void* dout = nullptr;
+  CEL_CUDA(c, cudaMallocAsync(&din, n * sizeof(double), c->stream));
+  CEL_CUDA(c, cudaMallocAsync(&dout, n * sizeof(double), c->stream));
+  CEL_CUDA(c, cudaMemcpyAsync(din, host_in, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  k_debug_math<<<(n + 255) / 256, 256, 0, c->stream>>>(which, (const double*)din, n, (double*)dout);
+  CEL_CUDA(c, cudaGetLastError());
+  CEL_CUDA(c, cudaMemcpyAsync(host_out, dout, n * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CEL_CUDA(c, cudaFreeAsync(din, c->stream));
+  CEL_CUDA(c, cudaFreeAsync(dout, c->stream));
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  return CEL_OK;
+}

@@ -235,6 +235,19 @@ __device__ __forceinline__ void draw_pair(const Params& P, uint32_t slot, uint32
   xb = to_uniform(o.w[2], o.w[3]);
 }
 
+// ---------------------------------------------------------------- small-angle trigonometry of the helix substep
+// sin x / x and (1 - cos x) / x^2 for |x| <= 0.5 (the helix angle of one chord substep, S7.3: h <= 0.5 / |omega|):
+// Taylor polynomials in y = x^2 <= 0.25, truncation < 1e-18; no argument reduction, no cancellation in 1 - cos
+__device__ __forceinline__ void sinc_versc_small(double y, double& S, double& V) {
+  double s = -1.0 / 1307674368000.0;                                 // -1/15!
+  s = fma(s, y, 1.0 / 6227020800.0); s = fma(s, y, -1.0 / 39916800.0); s = fma(s, y, 1.0 / 362880.0);
+  s = fma(s, y, -1.0 / 5040.0); s = fma(s, y, 1.0 / 120.0); s = fma(s, y, -1.0 / 6.0); s = fma(s, y, 1.0);
+  double v = 1.0 / 20922789888000.0;                                 // 1/16!
+  v = fma(v, y, -1.0 / 87178291200.0); v = fma(v, y, 1.0 / 479001600.0); v = fma(v, y, -1.0 / 3628800.0);
+  v = fma(v, y, 1.0 / 40320.0); v = fma(v, y, -1.0 / 720.0); v = fma(v, y, 1.0 / 24.0); v = fma(v, y, -0.5);
+  S = s; V = -v;
+}
+
 // ---------------------------------------------------------------- S4 table lookups
 struct GridPos { int j; double f; };
 __device__ __forceinline__ GridPos grid_locate(const Params& P, double E) {
@@ -403,11 +416,14 @@ __device__ __forceinline__ HelixFrame helix_frame(const Params& P, double dx, do
 }
 __device__ __forceinline__ void helix_point(const Params& P, const HelixFrame& F, double x, double y, double z, double omega, double h,
                                             double& ox, double& oy, double& oz, double& odx, double& ody, double& odz) {
-  double sn, cs;
-  sincos(omega * h, &sn, &cs);
-  double sh = sin(0.5 * omega * h);
-  double A = sn / omega;
-  double Bc = 2.0 * sh * sh / omega;
+  // sin(omega h)/omega = h S, 2 sin^2(omega h/2)/omega = (1 - cos(omega h))/omega = x h V with x = omega h, |x| <= 0.5
+  const double x_ = omega * h;
+  double S, V;
+  sinc_versc_small(x_ * x_, S, V);
+  const double sn = x_ * S;
+  const double cs = 1.0 - (x_ * x_) * V;
+  const double A = h * S;
+  const double Bc = (x_ * h) * V;
   odx = F.dpar * P.bhx + cs * F.px + sn * F.wx;
   ody = F.dpar * P.bhy + cs * F.py + sn * F.wy;
   odz = F.dpar * P.bhz + cs * F.pz + sn * F.wz;

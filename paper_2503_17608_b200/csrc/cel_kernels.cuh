@@ -536,6 +536,16 @@ __global__ void k_debug_uniforms(Params P, const uint32_t* slots, uint32_t n, ui
   out[i] = (j & 1u) ? xb : xa;
 }
 
+// which = 0: sin(x) of the helix substep (x S(x^2)); 1: 1 - cos(x) (x^2 V(x^2)), |x| <= 0.5
+__global__ void k_debug_math(int which, const double* in, uint32_t n, double* out) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double x = in[i];
+  double S, V;
+  sinc_versc_small(x * x, S, V);
+  out[i] = which == 0 ? x * S : (x * x) * V;
+}
+
 // every slot vacant: key byte 7 (padding 0xff), meta action VACANT (state bytes are otherwise zero); the per-tile
 // vacancy counters start at the number of real slots in the tile
 __global__ void k_reset_state(DeviceState D) {

@@ -101,6 +101,20 @@ def test_device_uniforms_bit_exact(binding):
     ctx.close()
 
 
+def test_device_elementary_functions(binding):
+    """the helix substep's small-angle sin and 1 - cos (Taylor polynomials, |x| <= 0.5: S7.3 bounds the angle of one
+    chord substep) agree with numpy's to a few ulp, so that first-step positions stay inside the 1e-12 bar"""
+    w = W.config1(n_events=1, n_slots=64)
+    ctx = binding.from_workload(w)
+    rng = np.random.default_rng(11)
+    x = np.concatenate([rng.uniform(-0.5, 0.5, 400000), rng.uniform(-1, 1, 100000) * 10.0 ** -rng.integers(1, 12, 100000), [0.0, 0.5, -0.5]])
+    s, v = ctx.debug_math(0, x), ctx.debug_math(1, x)
+    assert np.max(np.abs(s - np.sin(x)) / np.maximum(np.abs(np.sin(x)), 1e-300)) < 4.5e-16
+    ref = 2.0 * np.sin(0.5 * x) ** 2                     # the cancellation-free form of 1 - cos x (S7.3)
+    assert np.max(np.abs(v - ref) / np.maximum(ref, 1e-300)) < 9e-16
+    ctx.close()
+
+
 def test_device_tables_match_oracle(binding):
     w = W.config4(n_events=1, per_event=2, n_slots=64)
     ctx = binding.from_workload(w)
