@@ -400,7 +400,33 @@ int locate_primary(const Geometry& g, const double pos[3], const double dir[3]) 
 int64_t quantise(double x) { return (int64_t)std::llrint(x * TALLY_SCALE); }
 
 // ---------------------------------------------------------------- P1 init (S9)
+void load_initializer(OrcTrack& t, const Initializer& in) {
+  for (int i = 0; i < 3; ++i) { t.pos[i] = in.pos[i]; t.dir[i] = in.dir[i]; }
+  t.energy = in.energy; t.event = in.event; t.ptype = in.ptype;
+  t.vol = in.vol; t.surf = in.surf; t.nsteps = 0;
+  t.action = (in.ptype == GAMMA) ? MOVE_G : MOVE_C;
+}
+
+// S9-P (sort mode 3, section 3.2): the initializers popped in this iteration are partitioned by charge and
+// assigned to opposite ends of the track array: in pop order, the c-th charged one takes the c-th vacancy counted from
+// slot 0 upwards, the g-th neutral one the g-th vacancy counted from slot N-1 downwards.
+void phase_init_partition(Oracle& o) {
+  uint64_t I = o.init.size();
+  std::vector<uint64_t> vacant;
+  for (uint64_t s = 0; s < o.n_slots; ++s) if (o.tracks[s].action == VACANT) vacant.push_back(s);
+  uint64_t V = vacant.size();
+  uint64_t n_take = V < I ? V : I;
+  uint64_t c = 0, g = 0;
+  for (uint64_t j = 0; j < n_take; ++j) {
+    const Initializer& in = o.init[I - 1 - j];
+    uint64_t slot = (in.ptype == GAMMA) ? vacant[V - 1 - g++] : vacant[c++];
+    load_initializer(o.tracks[slot], in);
+  }
+  o.init.resize(I - n_take);
+}
+
 void phase_init(Oracle& o) {
+  if (o.sort_mode == 3) { phase_init_partition(o); return; }
   uint64_t I = o.init.size();
   uint64_t V = 0;
   for (uint64_t s = 0; s < o.n_slots; ++s) V += (o.tracks[s].action == VACANT);

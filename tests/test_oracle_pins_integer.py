@@ -91,6 +91,54 @@ def test_tiny_hand_checkable_fill():
     assert list(off) == [0, 0, 0, 0, 3, 3, 3, 3, 8]
 
 
+def test_partition_rule_hand_checkable():
+    """S9-P (section 3.2): N = 8, all vacant, primaries 0..4 = gamma, e-, e-, gamma, e+. Pop order is
+    init[4], init[3], ...: e+ -> lowest vacancy 0, gamma(3) -> highest vacancy 7, e-(2) -> 1, e-(1) -> 2, gamma(0) -> 6"""
+    w = W.config2(n_events=5, n_slots=8, sort_mode=3, energy=100.0)
+    w.primaries["ptype"] = [0, 1, 1, 0, 2]
+    w.primaries["energy"] = [10.0, 11.0, 12.0, 13.0, 14.0]
+    o = make_oracle(w)
+    o.begin(w.primaries, 5)
+    o.phase_init()
+    st = o.state()
+    assert list(st["energy"][[0, 1, 2, 6, 7]]) == [14.0, 12.0, 11.0, 10.0, 13.0]
+    assert list(st["ptype"][[0, 1, 2, 6, 7]]) == [2, 1, 1, 0, 0]
+    assert np.all(st["action"][3:6] == VACANT) and list(st["action"][[0, 1, 2, 6, 7]]) == [4, 4, 4, 3, 3]
+    assert len(o.initializers()) == 0
+
+
+def test_partition_rule_with_occupied_slots_and_starved_stack():
+    """vacancies {1, 2, 4, 5, 7} of 8 slots (V = 5) and 7 initializers: the top 5 are popped; charged ones climb from
+    the lowest vacancy, neutral ones descend from the highest, the other 2 stay on the stack in their order"""
+    w = W.config2(n_events=10, n_slots=8, sort_mode=3, energy=100.0)
+    w.primaries = w.primaries[:10].copy()
+    w.primaries["ptype"] = [1, 1, 1, 0, 1, 0, 0, 1, 0, 1]        # first 3 fill slots 0.. in a plain run below
+    w.primaries["energy"] = 20.0 + np.arange(10)
+    o = make_oracle(w)
+    o.begin(w.primaries, 10)
+    o.phase_init()                                                # 8 slots <- top 8 (ids 9..2); stack keeps ids 0, 1
+    st = o.state()
+    # pop order ids 9(c) 8(g) 7(c) 6(g) 5(g) 4(c) 3(g) 2(c): charged -> 0,1,2,3 ; neutral -> 7,6,5,4
+    assert list(st["energy"]) == [29.0, 27.0, 24.0, 22.0, 23.0, 25.0, 26.0, 28.0]
+    assert [int(e) for e in o.initializers()["energy"]] == [20, 21]
+
+
+def test_partition_mode_conserves_and_separates():
+    """same physics in every mode: per-event energy is conserved; from an empty array the charged tracks of the first
+    fill sit below every neutral one; a whole shower ends with the same number of histories' energy"""
+    w, o = small_shower(3, n_slots=512, n_events=5, energy=500.0, seed=33)
+    o.begin(w.primaries, w.n_events)
+    for _ in range(6):
+        o.step()
+        st = o.state()
+        ch = np.nonzero((st["action"] != VACANT) & (st["ptype"] != 0))[0]
+        ne = np.nonzero((st["action"] != VACANT) & (st["ptype"] == 0))[0]
+        if len(ch) and len(ne) and len(ch) + len(ne) < 200:      # far from full: no mixing yet
+            assert ch.max() < ne.min()
+    o.run()
+    assert np.abs(o.tallies().sum(1) - 500.0).max() < 1e-9 * 500.0
+
+
 def test_more_initializers_than_slots():
     w = W.config1(n_events=50, n_slots=16)
     o = make_oracle(w)
