@@ -29,7 +29,7 @@ if ROOT not in sys.path:
 
 from paper_2503_17608_b200 import workloads as W  # noqa: E402  (input data only)
 
-SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle"}
+SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle", 3: "partition"}
 ACTIONS = ("PE", "PAIR", "COMPTON", "MOVE_G", "MOVE_C", "BREMS", "ANNIH", "VACANT")
 STATE_BYTES = 64          # one slot's state: RecA + RecB
 INDEX_BYTES = 4
@@ -171,7 +171,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     counts: [iterations][8] action counts after P1. Returns {kernel name: bytes}."""
     c = counts.astype(np.float64).sum(0)
     it = float(len(counts))
-    idx = INDEX_BYTES if sort_mode != 0 else 0
+    idx = INDEX_BYTES if sort_mode in (1, 2) else 0
     rw = 2 * STATE_BYTES + idx          # gather + write back one slot through the index
     n = float(n_slots)
     sec = float(n_secondaries)
@@ -185,6 +185,11 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
         "charged": (c[4] + c[5]) * rw + c[5] * STATE_BYTES,                  # bremsstrahlung stages one photon
         "push": sec * (1 + 2 * STATE_BYTES),                                 # nsec byte + (read staging, write stack)
     }
+    # sort mode 3: two passes over the popped initializers (8 B meta each), 4 B pop position written, then read by the fill
+    out["part_count"] = float(n_initialised) * 8
+    out["part_scatter"] = float(n_initialised) * (8 + INDEX_BYTES)
+    if sort_mode == 3:
+        out["init_fill"] += float(n_initialised) * INDEX_BYTES
     # sorted by action the five action kernels are one launch (k_actions): the same bytes, summed
     out["actions"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair", "photon", "charged"))
     return out
@@ -340,7 +345,7 @@ def run_cuda(args):
     # ---- the other sort modes (BASELINE.json metric: per sort mode)
     per_mode = {}
     if not args.no_modes:
-        for mode in (0, 1, 2):
+        for mode in (0, 1, 2, 3):
             if mode == w.sort_mode:
                 per_mode[SORT_NAMES[mode]] = {"track_steps_per_s": track_steps / (ms * 1e-3) / world if world > 1 else track_steps / (ms * 1e-3),
                                               "events_per_s": w.n_events * args.steps / (ms * 1e-3)}
@@ -394,8 +399,8 @@ def main():
     ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4", "config5"])
     ap.add_argument("--events", type=int, default=0, help="override the workload's number of events")
     ap.add_argument("--slots", type=int, default=0, help="override the workload's number of track slots")
-    ap.add_argument("--sort-mode", type=int, default=1, choices=[0, 1, 2])
-    ap.add_argument("--no-modes", action="store_true", help="skip the other two sort modes")
+    ap.add_argument("--sort-mode", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--no-modes", action="store_true", help="skip the other sort modes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--oracle-events", type=int, default=200, help="events in the oracle's bounded sample")
     ap.add_argument("--oracle-slots", type=int, default=1 << 18)

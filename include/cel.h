@@ -24,7 +24,11 @@ extern "C" {
 
 typedef struct cel_ctx cel_ctx; /* opaque; owned by the library; freed by cel_destroy */
 
-enum { CEL_SORT_NONE = 0, CEL_SORT_BY_ACTION = 1, CEL_SORT_BY_PARTICLE = 2 };
+enum { CEL_SORT_NONE = 0, CEL_SORT_BY_ACTION = 1, CEL_SORT_BY_PARTICLE = 2,
+       /* PAPER.md:51 (section 3.2): no index array; the initializers popped in an iteration are partitioned by charge and
+        * assigned to opposite ends of the track array (docs/PHYSICS_SPEC.md S9-P): charged ones take the vacancies from
+        * slot 0 upwards, neutral ones from slot N-1 downwards; the kernels run masked over all slots as in mode NONE */
+       CEL_SORT_PARTITION = 3 };
 enum { CEL_GEOM_SLAB = 0, CEL_GEOM_CYL = 1 };
 enum { CEL_GAMMA = 0, CEL_ELECTRON = 1, CEL_POSITRON = 2 };
 /* action IDs = sort keys (docs/PHYSICS_SPEC.md S2) */
@@ -122,7 +126,9 @@ const char* cel_last_cuda_error(cel_ctx*);
  * P3i: ANNIH, PE, PAIR; P3i+P3m: PHOTON (Compton, then the photon move), CHARGED (bremsstrahlung, then the charged move
  * with energy loss and MSC); P4 (scoring) happens inside the action kernels; P5: PUSH. */
 enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
-       CEL_K_ACTIONS /* the five action kernels in one launch (sort by action, option fused) */, CEL_KERNEL_COUNT };
+       CEL_K_ACTIONS /* the five action kernels in one launch (sort by action, option fused) */,
+       CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
+       CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
 /* Per-kernel device time of the last transport run with option "profile" = 1 (per-kernel HBM

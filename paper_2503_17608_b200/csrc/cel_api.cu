@@ -253,7 +253,7 @@ extern "C" uint64_t cel_workspace_bytes(uint64_t n_slots, uint64_t init_capacity
 extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n_mats, const cel_physics* ph,
                           uint64_t n_slots, int sort_mode, cel_ctx** out) {
   if (!g || !mats || !ph || !out || n_mats < 1 || n_slots < 1 || n_slots > (1ull << 31)) return CEL_ERR_INVALID_ARG;
-  if (sort_mode < 0 || sort_mode > 2 || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
+  if (sort_mode < 0 || sort_mode > CEL_SORT_PARTITION || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
   if (g->n_vol < 1 || g->n_vol > 254 || !g->bounds || !g->vol_material || !g->vol_bin) return CEL_ERR_INVALID_ARG;
   for (int i = 0; i < g->n_vol; ++i) {
     if (!(g->bounds[i] < g->bounds[i + 1])) return CEL_ERR_INVALID_ARG;
@@ -435,7 +435,8 @@ int physics_grid(const cel_ctx* c) {
 }
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
-    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push", "actions"};
+    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push", "actions",
+    "part_count", "part_scatter"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
@@ -470,8 +471,12 @@ int enqueue_iteration_t(cel_ctx* c) {
   const bool cyl = D.P.geom_kind == CEL_GEOM_CYL, field = D.P.bmag != 0.0;
   int n = 0;
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1)], s);
+  if (D.sort_mode == CEL_SORT_PARTITION) {   // S9-P: the popped initializers are partitioned by charge before the fill
+    launch_chain(c, k_part_count<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_COUNT, n);
+    launch_chain(c, k_part_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_SCATTER, n);
+  }
   launch_chain(c, k_init_fill<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_INIT_FILL, n);
-  if (D.sort_mode != CEL_SORT_NONE) { launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n); }
+  if (D.sort_mode == CEL_SORT_BY_ACTION || D.sort_mode == CEL_SORT_BY_PARTICLE) { launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n); }
   if (D.sort_mode == CEL_SORT_BY_ACTION && c->fused) {
     // one launch walks the chunks of every action's range (k_actions): the whole iteration is one PDL chain
     if (cyl) { if (field) launch_chain(c, k_actions<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 1, TR>, pg, kBlock, s); }
@@ -536,6 +541,7 @@ const void* persistent_function(const cel_ctx* c) {
 void setup_persistent(cel_ctx* c) {
   c->persist_fn = persistent_function(c);
   c->persist_grid = 0;
+  if (c->D.sort_mode == CEL_SORT_PARTITION) return;   // the partition passes exist in the kernel-per-action form only
   int dev = 0, coop = 0, per_sm = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return;
   if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return;
@@ -567,7 +573,8 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   const uint64_t tiles = D.n_tiles;
   const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
   const uint64_t o_phist = align_up(o_hist + tiles * 32, 256);
-  const uint64_t scratch_bytes = align_up(o_phist + tiles * 32, 256);
+  const uint64_t o_part = align_up(o_phist + tiles * 32, 256);
+  const uint64_t scratch_bytes = align_up(o_part + tiles * 4, 256);
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
   const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
   CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));
@@ -575,6 +582,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   D.tile_hist = (uint32_t*)((char*)c->scratch + o_hist);
   D.tile_phist = (uint32_t*)((char*)c->scratch + o_phist);
   D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
+  D.part_cnt = (uint32_t*)((char*)c->scratch + o_part);
   D.tally = (unsigned long long*)c->d_tally;
   D.n_events = n_events;
   if (c->d_trace) { CEL_CUDA(c, cudaFreeAsync(c->d_trace, s)); c->d_trace = nullptr; }
@@ -828,7 +836,7 @@ extern "C" int cel_debug_read_indices(cel_ctx* c, uint32_t* idx, uint32_t* offse
   int rc = fetch_control(c);
   if (rc != CEL_OK) return rc;
   std::memcpy(offsets, c->last.offsets, 9 * sizeof(uint32_t));
-  if (c->D.sort_mode == CEL_SORT_NONE) {
+  if (c->D.sort_mode == CEL_SORT_NONE || c->D.sort_mode == CEL_SORT_PARTITION) {
     for (uint64_t i = 0; i < c->n_slots; ++i) idx[i] = (uint32_t)i;
   } else {
     CEL_CUDA(c, cudaMemcpyAsync(idx, c->D.indices, c->n_slots * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));

@@ -116,6 +116,7 @@ struct Control {
   uint32_t ticket_fill, ticket_push;
   uint32_t n_logged;
   uint32_t vac_total;               // V before the fill of this iteration
+  uint32_t part_charged;            // sort mode 3: charged initializers among the n_take popped in this iteration
   unsigned long long barrier;       // arrival counter of the persistent kernel's grid barrier (zeroed per launch)
 };
 
@@ -145,6 +146,7 @@ struct DeviceState {
   uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
   uint32_t* tile_hist;    // [n_tiles][8] per-tile action histogram (-> exclusive base per key after k_init_fill, sort by action)
   uint32_t* tile_phist;   // [n_tiles][8] per-tile particle histogram, 4 used (sort by particle)
+  uint32_t* part_cnt;     // [n_tiles] sort mode 3: charged pops per tile-sized chunk of the popped segment
   // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
   // in / last warp out of every kernel of every iteration; nullptr = off
   unsigned long long* trace;
@@ -153,7 +155,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_COUNT };
+enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_PART_COUNT, K_PART_SCATTER, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;

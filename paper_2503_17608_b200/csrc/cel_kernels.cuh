@@ -145,12 +145,28 @@ __device__ __forceinline__ uint32_t real_slots_in_tile(const DeviceState& D, uin
 // (`prefix`) is the sum of tile_vac over the tiles before it — scan-based, no atomics in the assignment, so the slot
 // assignment is deterministic. Adds the tile's action histogram to sm.act and (sort by particle) its
 // sort-key histogram to sm.hist; the caller zeroes both and synchronises before, and synchronises after.
-__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t n_take,
+// Which vacancies are filled: ranks [0, low_n) and [high_start, V). Plain rule (S9): low_n = n_take, high_start = V
+// (none at the high end), rank r takes pop position r. Partition rule (S9-P, sort mode 3): low_n = C charged,
+// high_start = V - G neutral; rank r < C takes the pop position plist[r], rank r >= V - G takes plist[n_take-1-(V-1-r)]
+// (plist = D.indices, written by k_part_scatter).
+struct FillPlan { uint32_t n_take, low_n, high_start, V; bool partition; };
+__device__ __forceinline__ FillPlan plain_plan(uint32_t n_take) { FillPlan p; p.n_take = n_take; p.low_n = n_take; p.high_start = 0xffffffffu; p.V = 0; p.partition = false; return p; }
+__device__ __forceinline__ FillPlan partition_plan(uint32_t n_take, uint32_t V, uint32_t n_charged) {
+  FillPlan p; p.n_take = n_take; p.low_n = n_charged; p.high_start = V - (n_take - n_charged); p.V = V; p.partition = true; return p;
+}
+// vacancies of ranks [prefix, prefix + v) that the plan fills
+__device__ __forceinline__ uint32_t filled_by_plan(uint32_t v, uint32_t prefix, const FillPlan& pl) {
+  const uint32_t end = prefix + v;
+  const uint32_t lo = min(end, pl.low_n) > prefix ? min(end, pl.low_n) - prefix : 0u;
+  const uint32_t hs = max(prefix, pl.high_start);
+  return lo + (end > hs ? end - hs : 0u);
+}
+__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, const FillPlan pl,
                                           uint32_t prefix, uint32_t tile_vacant) {
   uint32_t rank0 = prefix;                                   // rank of the first vacancy of the current sub-tile
   const uint32_t rank_end = prefix + tile_vacant;            // one past the rank of the tile's last vacancy
   const uint32_t real = real_slots_in_tile(D, tile);
-  if (tile_vacant == real && !(prefix < n_take)) {           // all vacant, nothing to fill: no key byte needs reading
+  if (tile_vacant == real && filled_by_plan(tile_vacant, prefix, pl) == 0) {   // all vacant, nothing to fill: no key byte needs reading
     if (threadIdx.x == 0) { atomicAdd(&sm.act[A_VACANT], real); if (D.sort_mode == 2) atomicAdd(&sm.hist[3], real); }
     return;
   }
@@ -159,7 +175,7 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
     const uint32_t sub_base = (tile << D.tile_shift) + sub * kSub;
     const uint32_t base = sub_base + threadIdx.x * kKeysPerThread;
     uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
-    if (rank0 < n_take && rank0 < rank_end) {               // block-uniform: this sub-tile may have vacancies to fill
+    if (rank0 < rank_end && filled_by_plan(rank_end - rank0, rank0, pl) != 0) {   // block-uniform: this sub-tile may have vacancies to fill
       const uint32_t c = count_vacant4(kv);
       uint32_t total;
       uint32_t r = block_excl_scan(c, sm.scan, total);
@@ -170,12 +186,19 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
           if (((kv >> (8 * i)) & 0xf) == A_VACANT) { sm.list[r] = base + i; ++r; }
       }
       __syncthreads();
-      const uint32_t nf = min(total, n_take - rank0);
+      // filled items of the sub-tile's list: [0, n_lo) at the low end of the ranks, [hi_begin, total) at the high end
+      const uint32_t n_lo = pl.low_n > rank0 ? min(total, pl.low_n - rank0) : 0u;
+      const uint32_t hi_begin = pl.high_start > rank0 ? min(total, pl.high_start - rank0) : 0u;
+      const uint32_t nf = n_lo + (total - hi_begin);
       // cooperative copy: work item w = (record, half); half 0 = RecA, half 1 = RecB (+ the key byte)
       for (uint32_t w = threadIdx.x; w < 2 * nf; w += kTileThreads) {
-        const uint32_t item = w >> 1;
+        const uint32_t m = w >> 1;
+        const uint32_t item = m < n_lo ? m : hi_begin + (m - n_lo);
         const uint32_t slot = sm.list[item];
-        const unsigned long long src = I - 1ull - (unsigned long long)(rank0 + item);
+        const uint32_t rank = rank0 + item;
+        uint32_t pop = rank;                                 // plain rule: rank r takes init[I-1-r]
+        if (pl.partition) pop = D.indices[rank < pl.low_n ? rank : pl.n_take - 1u - (pl.V - 1u - rank)];
+        const unsigned long long src = I - 1ull - (unsigned long long)pop;
         if (w & 1) {
           const RecB b = load_b(D.initB + src);
           store_b(D.stB + slot, b);
@@ -214,6 +237,10 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
       }
     }
   }
+}
+__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t n_take,
+                                          uint32_t prefix, uint32_t tile_vacant) {
+  fill_tile(D, sm, tile, I, plain_plan(n_take), prefix, tile_vacant);
 }
 // after fill_tile + __syncthreads: publish the tile's action histogram and (sort by particle) its sort-key histogram.
 // The iteration's action counts are the column sums of tile_hist (no same-address atomics from a thousand blocks).
@@ -413,7 +440,8 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   uint32_t prefix, V;
   block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);   // (its barriers also publish sm.hist / sm.act)
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
-  fill_tile(D, sm, tile, I, n_take, prefix, D.tile_vac[tile]);
+  const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, ctl->part_charged) : plain_plan(n_take);
+  fill_tile(D, sm, tile, I, plan, prefix, D.tile_vac[tile]);
   __syncthreads();
   publish_tile_hist(D, sm, tile);
   if (!last_block_done(&ctl->ticket_fill)) return;
@@ -429,7 +457,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
     uint32_t ex = block_excl_scan(sum, sm.scan, total);
 #pragma unroll
     for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) {
-      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - filled_in_tile(v[i], ex, n_take);
+      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - filled_by_plan(v[i], ex, plan);
       ex += v[i];
     }
   }
@@ -478,6 +506,80 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
       ctl->secondaries += S;
       ctl->iter += 1;
     }
+  }
+}
+
+// ================================================================ S9-P: charged / neutral partition of the popped initializers
+// (sort mode 3; section 3.2). Pop position j = 0 .. n_take-1 is init[I-1-j]. Two passes over the popped
+// segment, one tile-sized chunk per block: k_part_count counts the charged pops of a chunk; k_part_scatter forms the
+// chunk's exclusive prefix by a block reduction over the counts and writes the pop positions, stably, into
+// plist (= D.indices): the charged ones from the front in pop order, the neutral ones from the back.
+__device__ __forceinline__ bool pop_is_charged(const DeviceState& D, unsigned long long I, uint32_t j) {
+  const unsigned long long meta = reinterpret_cast<const unsigned long long*>(D.initB + (I - 1ull - j))[3];
+  return meta_ptype(meta) != P_GAMMA;
+}
+template <bool TRACE>
+__global__ void __launch_bounds__(kTileThreads) k_part_count(DeviceState D) {
+  __shared__ BookSmem sm;
+  pdl_prologue();
+  const Control* ctl = D.ctl;
+  if (ctl->finished) return;
+  const TraceScope<K_PART_COUNT, TRACE> trace(D, ctl->iter);
+  const uint32_t tile = blockIdx.x;
+  const unsigned long long I = ctl->n_init;
+  uint32_t prefix, V;
+  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);
+  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
+  const unsigned long long j0 = (unsigned long long)tile << D.tile_shift;
+  const unsigned long long j1 = min(j0 + (1ull << D.tile_shift), (unsigned long long)n_take);
+  uint32_t c = 0;
+  for (unsigned long long j = j0 + threadIdx.x; j < j1; j += kTileThreads) c += pop_is_charged(D, I, (uint32_t)j) ? 1u : 0u;
+  c = __reduce_add_sync(0xffffffffu, c);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sm.scan[threadIdx.x >> 5] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+    for (int w = 0; w < kTileThreads / 32; ++w) t += sm.scan[w];
+    D.part_cnt[tile] = t;
+  }
+}
+template <bool TRACE>
+__global__ void __launch_bounds__(kTileThreads) k_part_scatter(DeviceState D) {
+  __shared__ BookSmem sm;
+  pdl_prologue();
+  Control* ctl = D.ctl;
+  if (ctl->finished) return;
+  const TraceScope<K_PART_SCATTER, TRACE> trace(D, ctl->iter);
+  const uint32_t tile = blockIdx.x;
+  const unsigned long long I = ctl->n_init;
+  uint32_t prefix, V, cpre, C;
+  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);
+  __syncthreads();
+  block_prefix_total(D.part_cnt, D.n_tiles, tile, sm.scan, cpre, C);
+  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
+  if (tile == 0 && threadIdx.x == 0) ctl->part_charged = C;
+  const unsigned long long j0 = (unsigned long long)tile << D.tile_shift;
+  const unsigned long long j1 = min(j0 + (1ull << D.tile_shift), (unsigned long long)n_take);
+  for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
+    const unsigned long long base = j0 + (unsigned long long)sub * kSub + (unsigned long long)threadIdx.x * kKeysPerThread;
+    if (j0 + (unsigned long long)sub * kSub >= j1) break;           // block-uniform
+    bool ch[kKeysPerThread];
+    uint32_t c = 0;
+#pragma unroll
+    for (int i = 0; i < kKeysPerThread; ++i) { ch[i] = (base + i < j1) && pop_is_charged(D, I, (uint32_t)(base + i)); c += ch[i] ? 1u : 0u; }
+    uint32_t total;
+    uint32_t r = cpre + block_excl_scan(c, sm.scan, total);         // charged pops before this thread's first pop
+#pragma unroll
+    for (int i = 0; i < kKeysPerThread; ++i) {
+      const unsigned long long j = base + i;
+      if (j < j1) {
+        if (ch[i]) { D.indices[r] = (uint32_t)j; ++r; }
+        else D.indices[n_take - 1u - ((uint32_t)j - r)] = (uint32_t)j;   // neutral rank = j - (charged before j)
+      }
+    }
+    cpre += total;
+    __syncthreads();
   }
 }
 

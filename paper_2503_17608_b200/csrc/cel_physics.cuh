@@ -122,7 +122,7 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
   (void)k_iter; (void)P;                                                                                    \
   for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x)
 
-__device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode != 0) ? D.indices[tid] : tid; }
+__device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode == 1 || D.sort_mode == 2) ? D.indices[tid] : tid; }
 
 // S8 photoelectric: the photon's energy goes to an electron along d (or is deposited when electrons are local)
 __device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t slot, const RecA& a, const RecB& b) {

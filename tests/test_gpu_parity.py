@@ -126,14 +126,14 @@ def test_device_tables_match_oracle(binding):
     ctx.close()
 
 
-@pytest.mark.parametrize("sort_mode", [0, 1, 2])
+@pytest.mark.parametrize("sort_mode", [0, 1, 2, 3])
 def test_config1_lockstep_whole_run(binding, sort_mode):
     w = W.config1(n_events=1000, n_slots=4096, sort_mode=sort_mode)
     agreed = lockstep(binding, w, 40, must_match=2)
     assert agreed >= 2
 
 
-@pytest.mark.parametrize("sort_mode", [0, 1, 2])
+@pytest.mark.parametrize("sort_mode", [0, 1, 2, 3])
 def test_config1_ragged_and_oversubscribed(binding, sort_mode):
     # 1000 slots (not a multiple of the 4096-slot tile, nor of 16), 2500 primaries -> slot-starved init
     w = W.config1(n_events=2500, n_slots=1000, sort_mode=sort_mode)
@@ -141,7 +141,8 @@ def test_config1_ragged_and_oversubscribed(binding, sort_mode):
     assert agreed >= 3
 
 
-@pytest.mark.parametrize("cfg,sort_mode", [("calo", 1), ("calo_1T", 0), ("calo_1T", 1), ("calo_1T", 2), ("barrel", 1)])
+@pytest.mark.parametrize("cfg,sort_mode", [("calo", 1), ("calo_1T", 0), ("calo_1T", 1), ("calo_1T", 2), ("barrel", 1),
+                                           ("calo", 3), ("calo_1T", 3), ("barrel", 3)])
 def test_shower_lockstep_first_iterations(binding, cfg, sort_mode):
     """first-step per-track quantities to 1e-12 and integer work bit-exact; several tiles and a ragged tail"""
     if cfg == "calo":
@@ -213,6 +214,37 @@ def test_persistent_and_kernel_forms_identical(binding):
             assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
             assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
             assert a["kernel_launches"] < b["kernel_launches"]
+
+
+def test_partition_mode_whole_runs(binding):
+    """sort mode 3 (charged / neutral partition, section 3.2): whole showers conserve energy per event, are
+    reproducible bit for bit, keep the two species at opposite ends while the array is far from full, and follow the
+    oracle's run of the same mode closely (same seeds; only last-ulp decision flips separate them)"""
+    for w in (W.config3(n_events=30, n_slots=1 << 14, energy=2000.0, sort_mode=3), W.config4(n_events=2, per_event=6, n_slots=1 << 14, sort_mode=3)):
+        a, ca = run_gpu(binding, w, persistent=0)
+        b, cb = run_gpu(binding, w, persistent=0, use_graph=0, batch=5)
+        assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb)
+        e = a["fixed"].astype(np.float64).sum(1) * 2.0 ** -36
+        assert np.all(np.abs(e - expected_energy(w)) <= 1e-9 * expected_energy(w))
+        o = make_oracle(w)
+        o.transport(w.primaries, w.n_events)
+        c = o.counters()
+        assert abs(a["track_steps"] - c["track_steps"]) <= 0.02 * c["track_steps"]
+    # separation: step a young shower and look at the slots
+    w = W.config2(n_events=4, n_slots=1 << 13, energy=1000.0, sort_mode=3)
+    ctx = binding.from_workload(w)
+    ctx.begin(w.primaries, w.n_events)
+    seen = 0
+    for _ in range(12):
+        ctx.step()
+        st = ctx.state()
+        live = st["action"] != VACANT
+        ch, ne = np.nonzero(live & (st["ptype"] != 0))[0], np.nonzero(live & (st["ptype"] == 0))[0]
+        if len(ch) and len(ne) and len(ch) + len(ne) < (1 << 12):
+            assert ch.max() < ne.min()
+            seen += 1
+    assert seen >= 5
+    ctx.close()
 
 
 def test_fused_and_per_action_launches_identical(binding):
