@@ -144,8 +144,9 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * the run is slower). concurrent: 1 (default) = the independent action kernels of an iteration run as parallel
  * branches of the iteration graph; 0 = one after the other. pdl: programmatic dependent launch along the main
  * chain (default 1). persistent: the cooperative one-kernel form (default 0). fused: sorted by action, launch the
- * five action kernels as one grid that walks the chunks of every action's range (default 0 = one launch per
- * action on parallel graph branches; measured equal without a field, slower with one). trace: see cel_trace. */
+ * five action kernels as one grid that walks the chunks of every action's range; in the masked modes, one launch
+ * with one thread per slot and the action switched on (default 0 = one launch per action; DESIGN.md section 10 has the
+ * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). trace: see cel_trace. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a

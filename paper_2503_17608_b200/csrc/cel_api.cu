@@ -485,6 +485,13 @@ int enqueue_iteration_t(cel_ctx* c) {
     launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
     return n;
   }
+  if (c->fused) {   // masked modes: one launch, one thread per slot, the action switched on (k_actions_masked)
+    if (cyl) { if (field) launch_chain(c, k_actions_masked<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 1, TR>, pg, kBlock, s); }
+    else { if (field) launch_chain(c, k_actions_masked<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 0, TR>, pg, kBlock, s); }
+    after_launch(c, CEL_K_ACTIONS, n);
+    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    return n;
+  }
   const bool fork = c->concurrent && !c->profile;
   cudaStream_t s_photon = s, s_small = s;
   if (fork) {

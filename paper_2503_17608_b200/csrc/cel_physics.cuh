@@ -533,4 +533,33 @@ __global__ void __launch_bounds__(kBlock) k_actions(DeviceState D) {
   }
 }
 
+// ================================================================ all actions in ONE masked launch (modes none / by particle / partition)
+// One thread per slot of the kernel's range, the action read once and switched on: a slot is visited exactly once per
+// iteration, so no order between interaction and move kernels has to be kept, and the dense key bytes are read once
+// instead of once per action kernel. What it costs is what PAPER.md:37-47 describes: a warp whose lanes hold different
+// actions serialises their code paths — which the partition of sort mode 3 is there to reduce.
+// Results are bit-identical to the kernel-per-action form of the same sort mode.
+template <bool FIELD, int GEOM, bool TRACE>
+__global__ void __launch_bounds__(kBlock) k_actions_masked(DeviceState D) {
+  pdl_prologue();
+  const Control* ctl = D.ctl;
+  if (ctl->finished) return;
+  const uint32_t k_iter = ctl->iter;
+  const TraceScope<K_ACTIONS, TRACE> trace(D, k_iter);
+  // by particle: the non-vacant part of the index array (gamma | e- | e+); otherwise every slot
+  const uint32_t rb = 0, re = D.sort_mode == 2 ? ctl->offsets[3] : D.N;
+  for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x) {
+    const uint32_t slot = slot_of(D, tid);
+    if ((D.akey[slot] & 0xf) == A_VACANT) continue;
+    const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);
+    const int act = meta_action(b.meta);
+    if (act == A_MOVE_C || act == A_BREMS) do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
+    else if (act == A_MOVE_G || act == A_COMPTON) do_photon<GEOM>(D, slot, k_iter, a, b, act);
+    else if (act == A_PE) do_photoelectric(D, slot, a, b);
+    else if (act == A_PAIR) do_pair(D, slot, k_iter, a, b);
+    else if (act == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
+  }
+}
+
 }  // namespace cel

@@ -248,17 +248,18 @@ def test_partition_mode_whole_runs(binding):
 
 
 def test_fused_and_per_action_launches_identical(binding):
-    """sorted by action, the one-launch form (k_actions walks the chunks of every action's range) and the
-    launch-per-action form give the same tallies, per-iteration action counts and counters, bit for bit
-    (slab, slab + field, cylinder + field)"""
+    """the one-launch forms (sorted by action: k_actions walks the chunks of every action's range; masked modes:
+    k_actions_masked, one thread per slot with the action switched on) and the launch-per-action form give the same
+    tallies, per-iteration action counts and counters, bit for bit (slab, slab + field, cylinder + field)"""
     for w0 in (W.config2(n_events=20, n_slots=1 << 14, energy=3000.0), W.config3(n_events=20, n_slots=1 << 14, energy=3000.0),
                W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
-        w0.sort_mode = 1
-        a, ca = run_gpu(binding, w0, persistent=0, fused=1)
-        b, cb = run_gpu(binding, w0, persistent=0, fused=0)
-        assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), w0.name
-        assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
-        assert a["kernel_launches"] < b["kernel_launches"]
+        for mode in (1, 0, 2, 3):   # 1: k_actions over the action ranges; 0, 2, 3: k_actions_masked, one thread per slot
+            w0.sort_mode = mode
+            a, ca = run_gpu(binding, w0, persistent=0, fused=1)
+            b, cb = run_gpu(binding, w0, persistent=0, fused=0)
+            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
+            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
+            assert a["kernel_launches"] < b["kernel_launches"]
 
 
 def three_sigma(gt, ot):
