@@ -581,7 +581,9 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
   const uint64_t o_phist = align_up(o_hist + tiles * 32, 256);
   const uint64_t o_part = align_up(o_phist + tiles * 32, 256);
-  const uint64_t scratch_bytes = align_up(o_part + tiles * 4, 256);
+  const uint64_t o_group = align_up(o_part + tiles * 4, 256);
+  const uint64_t group_bytes = 2ull * kMaxGroups * 8 * sizeof(uint32_t);
+  const uint64_t scratch_bytes = align_up(o_group + 2 * group_bytes, 256);
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
   const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
   CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));
@@ -590,6 +592,8 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   D.tile_phist = (uint32_t*)((char*)c->scratch + o_phist);
   D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
   D.part_cnt = (uint32_t*)((char*)c->scratch + o_part);
+  D.group_hist = (uint32_t*)((char*)c->scratch + o_group);
+  D.group_phist = (uint32_t*)((char*)c->scratch + o_group + group_bytes);
   D.tally = (unsigned long long*)c->d_tally;
   D.n_events = n_events;
   if (c->d_trace) { CEL_CUDA(c, cudaFreeAsync(c->d_trace, s)); c->d_trace = nullptr; }

@@ -242,12 +242,35 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
                                           uint32_t prefix, uint32_t tile_vacant) {
   fill_tile(D, sm, tile, I, plain_plan(n_take), prefix, tile_vacant);
 }
+// Two-level histograms. Besides its own row tile_hist[tile][8], every fill block adds its counts into the row of its
+// GROUP of kGroupTiles tiles (integer atomics on 8 x n_groups addresses, double-buffered by the parity of the iteration:
+// the blocks of iteration k also zero the rows that iteration k+1 will add into). Column totals are then the sum of
+// <= 64 group rows, and the base of a tile in the counting sort is (groups before its group) + (tiles of its group
+// before it): 2 KB read by each scatter block, 2 KB by the one block that updates the control block — instead of one
+// block scanning all 32 KB of rows in place, which was 4.4 of the 12 us of an almost empty k_init_fill (one SM pulls
+// ~64 B per clock from L2; profiles/).
+constexpr int kGroupTiles = 32;
+constexpr int kMaxGroups = kMaxTiles / kGroupTiles;   // 64
+__device__ __forceinline__ uint32_t* group_rows(uint32_t* base, uint32_t parity) { return base + (size_t)parity * kMaxGroups * 8; }
 // after fill_tile + __syncthreads: publish the tile's action histogram and (sort by particle) its sort-key histogram.
 // The iteration's action counts are the column sums of tile_hist (no same-address atomics from a thousand blocks).
 __device__ __forceinline__ void publish_tile_hist(const DeviceState& D, BookSmem& sm, uint32_t tile) {
   if (threadIdx.x < 8) {
     D.tile_hist[tile * 8 + threadIdx.x] = sm.act[threadIdx.x];
     if (D.sort_mode == 2) D.tile_phist[tile * 8 + threadIdx.x] = threadIdx.x < 4 ? sm.hist[threadIdx.x] : 0u;
+  }
+}
+// the kernel-per-action form: the group rows of the two-level histograms (see group_rows)
+__device__ __forceinline__ void publish_group_hist(const DeviceState& D, BookSmem& sm, uint32_t tile, uint32_t parity) {
+  if (threadIdx.x < 8) {
+    const uint32_t g = tile / kGroupTiles;
+    const uint32_t a = sm.act[threadIdx.x];
+    if (a) atomicAdd(group_rows(D.group_hist, parity) + g * 8 + threadIdx.x, a);
+    if (D.sort_mode == 2 && threadIdx.x < 4) { const uint32_t h = sm.hist[threadIdx.x]; if (h) atomicAdd(group_rows(D.group_phist, parity) + g * 8 + threadIdx.x, h); }
+    if (tile < (uint32_t)kMaxGroups) {   // the rows the next iteration adds into (last read by the previous iteration's scatter)
+      group_rows(D.group_hist, parity ^ 1u)[tile * 8 + threadIdx.x] = 0u;
+      if (D.sort_mode == 2) group_rows(D.group_phist, parity ^ 1u)[tile * 8 + threadIdx.x] = 0u;
+    }
   }
 }
 // the rows the scatter takes its per-tile bases from: the action histogram (sort by action) or the particle histogram
@@ -289,6 +312,30 @@ __device__ __forceinline__ void scan_tile_rows(uint32_t* rows, uint32_t t0, uint
   }
   __syncthreads();
 }
+// sum over the rows r < n_rows (n_rows <= 32) of rows[r][0..8) by one warp; every lane gets the 8 column sums
+__device__ __forceinline__ void warp_sum_rows(const uint32_t* rows, uint32_t n_rows, uint32_t* out8) {
+  const uint32_t lane = threadIdx.x & 31;
+  uint4 a = make_uint4(0, 0, 0, 0), b = make_uint4(0, 0, 0, 0);
+  if (lane < n_rows) { a = *reinterpret_cast<const uint4*>(rows + lane * 8); b = *reinterpret_cast<const uint4*>(rows + lane * 8 + 4); }
+  out8[0] = __reduce_add_sync(0xffffffffu, a.x); out8[1] = __reduce_add_sync(0xffffffffu, a.y);
+  out8[2] = __reduce_add_sync(0xffffffffu, a.z); out8[3] = __reduce_add_sync(0xffffffffu, a.w);
+  out8[4] = __reduce_add_sync(0xffffffffu, b.x); out8[5] = __reduce_add_sync(0xffffffffu, b.y);
+  out8[6] = __reduce_add_sync(0xffffffffu, b.z); out8[7] = __reduce_add_sync(0xffffffffu, b.w);
+}
+// column totals of all groups (n_groups <= 64) into total[8] (shared) by warps 0 and 1; the caller synchronises after
+__device__ __forceinline__ void group_totals(const uint32_t* grows, uint32_t n_groups, uint32_t (*part)[8] /* shared [2][8] */) {
+  const uint32_t warp = threadIdx.x >> 5;
+  if (warp < 2) {
+    uint32_t s8[8];
+    const uint32_t first = warp * 32;
+    warp_sum_rows(grows + (size_t)first * 8, n_groups > first ? min(32u, n_groups - first) : 0u, s8);
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) part[warp][k] = s8[k];
+    }
+  }
+}
+
 // vacancies of a tile that the fill of this iteration takes: min(v, max(0, n_take - (vacancies before the tile)))
 __device__ __forceinline__ uint32_t filled_in_tile(uint32_t v, uint32_t prefix, uint32_t n_take) {
   return min(v, n_take > prefix ? n_take - prefix : 0u);
@@ -425,8 +472,8 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
 }
 
 // ================================================================ the bookkeeping kernels (one block per tile)
-// k_init_fill: P1 + the per-tile histograms; its last block turns the histograms into per-key bases (exclusive scan
-// over the tiles), takes the filled vacancies off tile_vac, and updates offsets, ranges, counters and the log.
+// k_init_fill: P1 + the per-tile and per-group histograms; its last block takes the filled vacancies off tile_vac, sums
+// the group rows into the iteration's counts and updates offsets, ranges, counters and the log.
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
@@ -444,6 +491,8 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   fill_tile(D, sm, tile, I, plan, prefix, D.tile_vac[tile]);
   __syncthreads();
   publish_tile_hist(D, sm, tile);
+  const uint32_t parity = ctl->iter & 1u;
+  publish_group_hist(D, sm, tile, parity);
   if (!last_block_done(&ctl->ticket_fill)) return;
   // ---- last block: thread t owns `per` consecutive tiles
   const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;   // <= kMaxTiles / 256 = 8
@@ -461,14 +510,18 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
       ex += v[i];
     }
   }
-  // column sums of the action histogram = the iteration's action counts; exclusive scan over the tiles of the rows the
-  // scatter uses (in place)
-  __shared__ uint32_t act_total[8], key_total[8];
-  __shared__ uint32_t warp_tot[kTileThreads / 32][8];
+  // column sums of the group rows = the iteration's action counts (and sort-key counts)
+  __shared__ uint32_t act_part[2][8], key_part[2][8];
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
-  scan_tile_rows(D.tile_hist, t0, t1, D.sort_mode == 1, warp_tot, act_total);
-  if (D.sort_mode == 2) scan_tile_rows(D.tile_phist, t0, t1, true, warp_tot, key_total);
-  if (threadIdx.x == 0) update_control_after_fill(D, act_total, D.sort_mode == 2 ? key_total : act_total, n_keys, I, V, n_take);
+  const uint32_t n_groups = (D.n_tiles + kGroupTiles - 1) / kGroupTiles;
+  group_totals(group_rows(D.group_hist, parity), n_groups, act_part);
+  if (D.sort_mode == 2) group_totals(group_rows(D.group_phist, parity), n_groups, key_part);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t act_total[8], key_total[8];
+    for (int k = 0; k < 8; ++k) { act_total[k] = act_part[0][k] + act_part[1][k]; key_total[k] = D.sort_mode == 2 ? key_part[0][k] + key_part[1][k] : act_total[k]; }
+    update_control_after_fill(D, act_total, key_total, n_keys, I, V, n_take);
+  }
 }
 
 template <bool TRACE>
@@ -479,7 +532,23 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   if (ctl->finished) return;
   const TraceScope<K_SCATTER, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
-  if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + sort_rows(D)[tile * 8 + threadIdx.x];
+  {  // base[key] = offset[key] + (groups before the tile's group)[key] + (tiles of the group before the tile)[key]
+    const uint32_t parity = ctl->iter & 1u;
+    const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5;
+    __shared__ uint32_t part[3][8];
+    if (warp < 3) {
+      uint32_t s8[8];
+      const uint32_t* grows = group_rows(D.sort_mode == 2 ? D.group_phist : D.group_hist, parity);
+      if (warp < 2) warp_sum_rows(grows + (size_t)warp * 32 * 8, g > warp * 32 ? min(32u, g - warp * 32) : 0u, s8);
+      else warp_sum_rows(sort_rows(D) + (size_t)g * kGroupTiles * 8, tile - g * kGroupTiles, s8);
+      if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) part[warp][k] = s8[k];
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + part[0][threadIdx.x] + part[1][threadIdx.x] + part[2][threadIdx.x];
+  }
   __syncthreads();
   scatter_tile(D, sm, tile, D.tile_vac[tile]);
 }
