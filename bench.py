@@ -33,6 +33,7 @@ SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle", 3: "partition"}
 ACTIONS = ("PE", "PAIR", "COMPTON", "MOVE_G", "MOVE_C", "BREMS", "ANNIH", "VACANT")
 STATE_BYTES = 64          # one slot's state: RecA + RecB
 INDEX_BYTES = 4
+MAX_SUBSTEPS = 0        # --max-substeps: 0 = the workload's own (10)
 
 
 def make_workload(name, n_events, n_slots, sort_mode, seed_offset=0):
@@ -48,6 +49,9 @@ def make_workload(name, n_events, n_slots, sort_mode, seed_offset=0):
         w = W.config5(n_events=n_events or 2000, n_slots=n_slots or (1 << 20), sort_mode=sort_mode, seed=5 + seed_offset)
     else:
         raise SystemExit(f"unknown workload {name}")
+    if MAX_SUBSTEPS:
+        w.physics["max_substeps"] = MAX_SUBSTEPS       # PAPER.md:57 (fig. 1): the cap on chord substeps per iteration
+        w.notes += f", max_substeps {MAX_SUBSTEPS}"
     return w
 
 
@@ -404,7 +408,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--oracle-events", type=int, default=200, help="events in the oracle's bounded sample")
     ap.add_argument("--oracle-slots", type=int, default=1 << 18)
+    ap.add_argument("--max-substeps", type=int, default=0, help="override the cap on helix chord substeps per iteration (PAPER.md:57)")
     args = ap.parse_args()
+    global MAX_SUBSTEPS
+    MAX_SUBSTEPS = args.max_substeps
     if args.warmup < 3 and args.impl == "cuda":
         print("bench.py: warning: fewer than 3 warm-up steps", file=sys.stderr)
     return run_reference(args) if args.impl == "reference" else run_cuda(args)
