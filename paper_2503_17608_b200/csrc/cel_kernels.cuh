@@ -99,6 +99,36 @@ __device__ __forceinline__ void block_prefix_total(const uint32_t* a, uint32_t n
   for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
   prefix = p; total = t;
 }
+// The same with the counters already in registers: load_counters issues every load of the kernel's prologue back to
+// back (control block, counters) BEFORE the first use, so the prologue costs one L2 round trip instead of one per
+// dependent step (in-order issue stalls at the first use). Also returns a[tile].
+constexpr int kCountersPerThread = kMaxTiles / kTileThreads;   // 8
+__device__ __forceinline__ void load_counters(const uint32_t* a, uint32_t n, uint32_t (&v)[kCountersPerThread]) {
+#pragma unroll
+  for (int i = 0; i < kCountersPerThread; ++i) { const uint32_t idx = threadIdx.x + i * kTileThreads; v[i] = idx < n ? a[idx] : 0u; }
+}
+__device__ __forceinline__ void block_prefix_total_regs(const uint32_t (&v)[kCountersPerThread], uint32_t tile, uint32_t* smem /* 19 words */,
+                                                        uint32_t& prefix, uint32_t& total, uint32_t& own) {
+  uint32_t p = 0, t = 0;
+#pragma unroll
+  for (int i = 0; i < kCountersPerThread; ++i) {
+    const uint32_t idx = threadIdx.x + i * kTileThreads;
+    t += v[i];
+    if (idx < tile) p += v[i];
+  }
+  p = __reduce_add_sync(0xffffffffu, p);
+  t = __reduce_add_sync(0xffffffffu, t);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();
+  if (lane == 0) { smem[warp] = p; smem[9 + warp] = t; }
+#pragma unroll
+  for (int i = 0; i < kCountersPerThread; ++i) if (threadIdx.x + i * kTileThreads == tile) smem[18] = v[i];
+  __syncthreads();
+  p = 0; t = 0;
+#pragma unroll
+  for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
+  prefix = p; total = t; own = smem[18];
+}
 // "last block done" ticket: true in exactly one block, after every other block's global writes are visible
 __device__ __forceinline__ bool last_block_done(uint32_t* ticket) {
   __shared__ bool is_last;
@@ -128,7 +158,7 @@ __device__ __forceinline__ uint32_t count_vacant4(uint32_t w) {
 
 // ---------------------------------------------------------------- shared memory of a bookkeeping block
 struct BookSmem {
-  uint32_t scan[18];
+  uint32_t scan[20];
   unsigned long long scan64[9];
   uint32_t hist[8], act[8], base[8];
   uint32_t skey[kTileThreads];   // the sub-tile's key bytes
@@ -479,19 +509,23 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const TraceScope<K_INIT_FILL, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
+  // every load of the prologue is issued before the first use
+  const uint32_t finished = ctl->finished, iter = ctl->iter, n_charged = ctl->part_charged;
   const unsigned long long I = ctl->n_init;
+  uint32_t cnt[kCountersPerThread];
+  load_counters(D.tile_vac, D.n_tiles, cnt);
+  if (finished) return;
+  const TraceScope<K_INIT_FILL, TRACE> trace(D, iter);
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
-  uint32_t prefix, V;
-  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);   // (its barriers also publish sm.hist / sm.act)
+  uint32_t prefix, V, tile_vacant;
+  block_prefix_total_regs(cnt, tile, sm.scan, prefix, V, tile_vacant);   // (its barriers also publish sm.hist / sm.act)
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
-  const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, ctl->part_charged) : plain_plan(n_take);
-  fill_tile(D, sm, tile, I, plan, prefix, D.tile_vac[tile]);
+  const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
+  fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
   __syncthreads();
   publish_tile_hist(D, sm, tile);
-  const uint32_t parity = ctl->iter & 1u;
+  const uint32_t parity = iter & 1u;
   publish_group_hist(D, sm, tile, parity);
   if (!last_block_done(&ctl->ticket_fill)) return;
   // ---- last block: thread t owns `per` consecutive tiles
@@ -529,11 +563,14 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   const Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const TraceScope<K_SCATTER, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
+  const uint32_t finished = ctl->finished, iter = ctl->iter;
+  const uint32_t tile_vacant = D.tile_vac[tile];
+  const uint32_t my_offset = threadIdx.x < 8 ? ctl->offsets[threadIdx.x] : 0u;
+  if (finished) return;
+  const TraceScope<K_SCATTER, TRACE> trace(D, iter);
   {  // base[key] = offset[key] + (groups before the tile's group)[key] + (tiles of the group before the tile)[key]
-    const uint32_t parity = ctl->iter & 1u;
+    const uint32_t parity = iter & 1u;
     const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5;
     __shared__ uint32_t part[3][8];
     if (warp < 3) {
@@ -547,10 +584,10 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
       }
     }
     __syncthreads();
-    if (threadIdx.x < 8) sm.base[threadIdx.x] = ctl->offsets[threadIdx.x] + part[0][threadIdx.x] + part[1][threadIdx.x] + part[2][threadIdx.x];
+    if (threadIdx.x < 8) sm.base[threadIdx.x] = my_offset + part[0][threadIdx.x] + part[1][threadIdx.x] + part[2][threadIdx.x];
   }
   __syncthreads();
-  scatter_tile(D, sm, tile, D.tile_vac[tile]);
+  scatter_tile(D, sm, tile, tile_vacant);
 }
 
 template <bool TRACE>
@@ -558,22 +595,26 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const TraceScope<K_PUSH, TRACE> trace(D, ctl->iter);
   const uint32_t tile = blockIdx.x;
+  const uint32_t finished = ctl->finished, iter = ctl->iter;
+  const int32_t error = ctl->error;
   const unsigned long long I = ctl->n_init;
-  uint32_t prefix, S;
-  block_prefix_total(D.tile_sec, D.n_tiles, tile, sm.scan, prefix, S);
-  const bool overflow = ctl->error != 0 || I + S > D.init_capacity;
-  push_tile(D, sm, tile, I, prefix, D.tile_sec[tile], overflow);
+  uint32_t cnt[kCountersPerThread];
+  load_counters(D.tile_sec, D.n_tiles, cnt);
+  if (finished) return;
+  const TraceScope<K_PUSH, TRACE> trace(D, iter);
+  uint32_t prefix, S, tile_total;
+  block_prefix_total_regs(cnt, tile, sm.scan, prefix, S, tile_total);
+  const bool overflow = error != 0 || I + S > D.init_capacity;
+  push_tile(D, sm, tile, I, prefix, tile_total, overflow);
   if (last_block_done(&ctl->ticket_push)) {
     for (uint32_t i = threadIdx.x; i < D.n_tiles; i += kTileThreads) D.tile_sec[i] = 0;
     if (threadIdx.x == 0) {
       ctl->push_total = S;
       if (I + S > D.init_capacity) ctl->error = -4;  // CEL_ERR_INIT_OVERFLOW (sticky)
-      else if (ctl->error == 0) ctl->n_init = I + S;
+      else if (error == 0) ctl->n_init = I + S;
       ctl->secondaries += S;
-      ctl->iter += 1;
+      ctl->iter = iter + 1;
     }
   }
 }

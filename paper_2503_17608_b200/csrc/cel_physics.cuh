@@ -114,9 +114,10 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 #define CEL_FOR_RANGE(RANGE_ID, KERNEL_ID)                                                                  \
   pdl_prologue();                                                                                           \
   const Control* ctl = D.ctl;                                                                               \
-  if (ctl->finished) return;                                                                                \
+  const uint32_t finished_ = ctl->finished;   /* the four loads are issued together: one round trip */      \
   const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
   const uint32_t k_iter = ctl->iter;                                                                        \
+  if (finished_) return;                                                                                    \
   const TraceScope<KERNEL_ID, TRACE> trace(D, k_iter);                                                      \
   const Params& P = D.P;                                                                                    \
   (void)k_iter; (void)P;                                                                                    \
