@@ -26,7 +26,7 @@ namespace {
 constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action counts are logged
 constexpr int kStatusSlots = 2;
 constexpr int kMaxKernelsPerIteration = 16;
-constexpr int kSideStreams = 2;
+constexpr int kSideStreams = 4;
 
 struct HostTables {                 // per material, kept for cel_debug_table
   std::vector<double> t[5];         // compton, pe, pair, brems, range
@@ -50,8 +50,8 @@ struct cel_ctx {
   // stream-ordered scratch of the current run
   void* scratch = nullptr; void* d_tally = nullptr; void* d_prim = nullptr;
   cudaStream_t stream = nullptr; bool own_stream = false;
-  cudaStream_t side[kSideStreams] = {nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
-  cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr};
+  cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
+  cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
   int fused = 0;   // sort by action: all action kernels in one launch (k_actions); measured equal (no field) to 6 % slower (field)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
@@ -493,31 +493,30 @@ int enqueue_iteration_t(cel_ctx* c) {
     return n;
   }
   const bool fork = c->concurrent && !c->profile;
-  cudaStream_t s_photon = s, s_small = s;
+  const bool by_action = D.sort_mode == CEL_SORT_BY_ACTION;
+  // sorted by action: photon, annihilation, photoelectric, pair on one branch each (their ranges are disjoint and fixed);
+  // masked modes: {photoelectric -> pair -> photon} on one branch beside {annihilation -> charged} on the main stream
+  cudaStream_t s_photon = s, s_annih = s, s_pe = s, s_pair = s;
+  int n_side = 0;
   if (fork) {
+    n_side = by_action ? 4 : 1;
     cudaEventRecord(c->ev_fork, s);
-    cudaStreamWaitEvent(c->side[0], c->ev_fork, 0);
-    s_photon = c->side[0]; s_small = c->side[0];
-    if (D.sort_mode == CEL_SORT_BY_ACTION) { cudaStreamWaitEvent(c->side[1], c->ev_fork, 0); s_small = c->side[1]; }
+    for (int i = 0; i < n_side; ++i) cudaStreamWaitEvent(c->side[i], c->ev_fork, 0);
+    s_photon = c->side[0]; s_pe = c->side[0]; s_pair = c->side[0];
+    if (by_action) { s_annih = c->side[1]; s_pe = c->side[2]; s_pair = c->side[3]; }
   }
-  // chain on the main stream: annihilation (must precede the charged kernel in the masked modes), charged
-  cudaStream_t s_annih = (fork && D.sort_mode == CEL_SORT_BY_ACTION) ? s_small : s;
   if (c->phys.enable_annihilation) { k_annihilation<TR><<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
-  k_photoelectric<TR><<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PE, n);
-  if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_small>>>(D); after_launch(c, CEL_K_PAIR, n); }
+  k_photoelectric<TR><<<pg, kBlock, 0, s_pe>>>(D); after_launch(c, CEL_K_PE, n);
+  if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_pair>>>(D); after_launch(c, CEL_K_PAIR, n); }
   if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
   after_launch(c, CEL_K_PHOTON, n);
   // (in the masked modes the annihilation kernel precedes it on the main stream)
   if (cyl) { if (field) launch_chain(c, k_charged<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 1, TR>, pg, kBlock, s); }
   else { if (field) launch_chain(c, k_charged<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 0, TR>, pg, kBlock, s); }
   after_launch(c, CEL_K_CHARGED, n);
-  if (fork) {
-    cudaEventRecord(c->ev_join[0], c->side[0]);
-    cudaStreamWaitEvent(s, c->ev_join[0], 0);
-    if (D.sort_mode == CEL_SORT_BY_ACTION) {
-      cudaEventRecord(c->ev_join[1], c->side[1]);
-      cudaStreamWaitEvent(s, c->ev_join[1], 0);
-    }
+  for (int i = 0; i < n_side; ++i) {
+    cudaEventRecord(c->ev_join[i], c->side[i]);
+    cudaStreamWaitEvent(s, c->ev_join[i], 0);
   }
   launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
   return n;
