@@ -196,6 +196,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
         out["init_fill"] += float(n_initialised) * INDEX_BYTES
     # sorted by action the five action kernels are one launch (k_actions): the same bytes, summed
     out["actions"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair", "photon", "charged"))
+    out["discrete"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair"))
     return out
 
 
@@ -337,7 +338,7 @@ def run_cuda(args):
     dk = kernels[dominant]
     traffic, traffic_it = load_profile_traffic(dominant)
     alg_at_it = None
-    if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "actions"):
+    if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "actions", "discrete"):
         alg_at_it = algorithmic_bytes(counts[traffic_it:traffic_it + 1], w.n_slots, w.sort_mode, 0, 0)[dominant]
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": dk["frac"], "traffic": traffic, "traffic_iteration": traffic_it,

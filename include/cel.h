@@ -128,6 +128,7 @@ const char* cel_last_cuda_error(cel_ctx*);
 enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
        CEL_K_ACTIONS /* the five action kernels in one launch (sort by action, option fused) */,
        CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
+       CEL_K_DISCRETE /* photoelectric + pair + annihilation in one launch (sort by action, option merge_discrete) */,
        CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
@@ -146,7 +147,8 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * chain (default 1). persistent: the cooperative one-kernel form (default 0). fused: sorted by action, launch the
  * five action kernels as one grid that walks the chunks of every action's range; in the masked modes, one launch
  * with one thread per slot and the action switched on (default 0 = one launch per action; DESIGN.md section 10 has the
- * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). trace: see cel_trace. */
+ * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). merge_discrete: sorted by action, photoelectric + pair + annihilation
+ * in one launch (default 1). trace: see cel_trace. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a

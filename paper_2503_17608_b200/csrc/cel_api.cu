@@ -53,6 +53,7 @@ struct cel_ctx {
   cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
   cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
+  int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   int fused = 0;   // sort by action: all action kernels in one launch (k_actions); measured equal (no field) to 6 % slower (field)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
@@ -61,7 +62,7 @@ struct cel_ctx {
   void* h_prim = nullptr; size_t h_prim_bytes = 0;         // pinned staging of primaries
   cudaGraph_t graph = nullptr; cudaGraphExec_t graph_exec = nullptr;
   int trace_iters = 0; int trace_ends = 1; void* d_trace = nullptr;   // option "trace": device-side timeline of the first trace_iters iterations
-  DeviceState graph_D{}; int graph_cfg[5] = {-1, -1, -1, -1, -1};   // what the captured graph has baked in (arguments, options)
+  DeviceState graph_D{}; int graph_cfg[6] = {-1, -1, -1, -1, -1, -1};   // what the captured graph has baked in (arguments, options)
   int use_graph = 1; int batch = 16; int64_t max_iterations = 1ll << 22;
   int persistent = 0; int persist_batch = 64;   // one cooperative kernel runs up to persist_batch iterations
   int persist_grid = 0;                         // co-resident blocks of k_persistent (0 = not available)
@@ -401,6 +402,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "persistent")) c->persistent = v ? 1 : 0;
   else if (!std::strcmp(name, "pdl")) c->pdl = v ? 1 : 0;
   else if (!std::strcmp(name, "fused")) c->fused = v ? 1 : 0;
+  else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
   else if (!std::strcmp(name, "persist_batch")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->persist_batch = (int)v; }
@@ -436,7 +438,7 @@ int physics_grid(const cel_ctx* c) {
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
     "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push", "actions",
-    "part_count", "part_scatter"};
+    "part_count", "part_scatter", "discrete"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
@@ -499,15 +501,20 @@ int enqueue_iteration_t(cel_ctx* c) {
   cudaStream_t s_photon = s, s_annih = s, s_pe = s, s_pair = s;
   int n_side = 0;
   if (fork) {
-    n_side = by_action ? 4 : 1;
+    n_side = by_action ? (c->merge_discrete ? 2 : 4) : 1;
     cudaEventRecord(c->ev_fork, s);
     for (int i = 0; i < n_side; ++i) cudaStreamWaitEvent(c->side[i], c->ev_fork, 0);
     s_photon = c->side[0]; s_pe = c->side[0]; s_pair = c->side[0];
     if (by_action) { s_annih = c->side[1]; s_pe = c->side[2]; s_pair = c->side[3]; }
   }
-  if (c->phys.enable_annihilation) { k_annihilation<TR><<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
-  k_photoelectric<TR><<<pg, kBlock, 0, s_pe>>>(D); after_launch(c, CEL_K_PE, n);
-  if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_pair>>>(D); after_launch(c, CEL_K_PAIR, n); }
+  if (by_action && c->merge_discrete) {
+    const int dg = pg < 2 * c->n_sm ? pg : 2 * c->n_sm;
+    k_discrete<TR><<<dg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_DISCRETE, n);
+  } else {
+    if (c->phys.enable_annihilation) { k_annihilation<TR><<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
+    k_photoelectric<TR><<<pg, kBlock, 0, s_pe>>>(D); after_launch(c, CEL_K_PE, n);
+    if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_pair>>>(D); after_launch(c, CEL_K_PAIR, n); }
+  }
   if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
   after_launch(c, CEL_K_PHOTON, n);
   // (in the masked modes the annihilation kernel precedes it on the main stream)
@@ -621,7 +628,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
   // (the stream-ordered pool hands the same scratch back run after run, so the graph of the last run is normally
   // still valid: it is kept when every baked-in argument and option is unchanged)
-  const int cfg[5] = {c->batch, c->concurrent, c->pdl, c->fused, c->trace_iters};
+  const int cfg[6] = {c->batch, c->concurrent, c->pdl, c->fused, c->trace_iters, c->merge_discrete};
   const bool graph_valid = c->graph_exec && std::memcmp(&c->graph_D, &D, sizeof(DeviceState)) == 0 &&
                            std::memcmp(c->graph_cfg, cfg, sizeof(cfg)) == 0;
   if (!graph_valid) {

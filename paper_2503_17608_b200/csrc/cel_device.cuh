@@ -157,7 +157,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_PART_COUNT, K_PART_SCATTER, K_COUNT };
+enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;

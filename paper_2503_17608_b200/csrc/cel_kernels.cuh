@@ -507,19 +507,23 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
-  pdl_prologue();
   Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
-  // every load of the prologue is issued before the first use
-  const uint32_t finished = ctl->finished, iter = ctl->iter, n_charged = ctl->part_charged;
-  const unsigned long long I = ctl->n_init;
+  // Before the programmatic-dependency wait: what does NOT depend on the kernel just before this one in the stream
+  // (k_push of the previous iteration, or the partition passes, which only touch the stack, its height, `iter` and
+  // plist): the vacancy counters and `finished` were last written by the action kernels / the previous k_init_fill,
+  // which had completed before that kernel let this one start. The vacancy prefix so overlaps the push.
+  const uint32_t finished = ctl->finished;
   uint32_t cnt[kCountersPerThread];
   load_counters(D.tile_vac, D.n_tiles, cnt);
-  if (finished) return;
-  const TraceScope<K_INIT_FILL, TRACE> trace(D, iter);
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
   uint32_t prefix, V, tile_vacant;
   block_prefix_total_regs(cnt, tile, sm.scan, prefix, V, tile_vacant);   // (its barriers also publish sm.hist / sm.act)
+  pdl_prologue();
+  const uint32_t iter = ctl->iter, n_charged = ctl->part_charged;
+  const unsigned long long I = ctl->n_init;
+  if (finished) return;
+  const TraceScope<K_INIT_FILL, TRACE> trace(D, iter);
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
   fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
