@@ -47,6 +47,7 @@ def test_timeline_is_ordered_and_does_not_change_results(binding):
     ref = ctx.tallies_view()
     ref_fixed = ref["fixed"].copy()
     ctx.set_option("trace", 64)
+    ctx.set_option("merge_discrete", 0)      # one launch per action, so that every action kernel has its own stamps
     ctx.transport(w.primaries, w.n_events)
     v = ctx.tallies_view()
     assert np.array_equal(v["fixed"], ref_fixed) and v["track_steps"] == ref["track_steps"]
