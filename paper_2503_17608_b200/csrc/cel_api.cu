@@ -402,7 +402,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "persistent")) c->persistent = v ? 1 : 0;
   else if (!std::strcmp(name, "pdl")) c->pdl = v ? 1 : 0;
   else if (!std::strcmp(name, "fused")) c->fused = v ? 1 : 0;
-  else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
+  else if (!std::strcmp(name, "merge_discrete")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->merge_discrete = (int)v; }
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
   else if (!std::strcmp(name, "persist_batch")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->persist_batch = (int)v; }
@@ -501,13 +501,17 @@ int enqueue_iteration_t(cel_ctx* c) {
   cudaStream_t s_photon = s, s_annih = s, s_pe = s, s_pair = s;
   int n_side = 0;
   if (fork) {
-    n_side = by_action ? (c->merge_discrete ? 2 : 4) : 1;
+    n_side = by_action ? (c->merge_discrete == 2 ? 1 : (c->merge_discrete ? 2 : 4)) : 1;
     cudaEventRecord(c->ev_fork, s);
     for (int i = 0; i < n_side; ++i) cudaStreamWaitEvent(c->side[i], c->ev_fork, 0);
     s_photon = c->side[0]; s_pe = c->side[0]; s_pair = c->side[0];
     if (by_action) { s_annih = c->side[1]; s_pe = c->side[2]; s_pair = c->side[3]; }
   }
-  if (by_action && c->merge_discrete) {
+  const bool merge_photon = by_action && c->merge_discrete == 2;
+  if (merge_photon) {
+    if (cyl) k_neutral<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_neutral<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
+    after_launch(c, CEL_K_DISCRETE, n);
+  } else if (by_action && c->merge_discrete) {
     const int dg = pg < 2 * c->n_sm ? pg : 2 * c->n_sm;
     k_discrete<TR><<<dg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_DISCRETE, n);
   } else {
@@ -515,8 +519,10 @@ int enqueue_iteration_t(cel_ctx* c) {
     k_photoelectric<TR><<<pg, kBlock, 0, s_pe>>>(D); after_launch(c, CEL_K_PE, n);
     if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_pair>>>(D); after_launch(c, CEL_K_PAIR, n); }
   }
-  if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
-  after_launch(c, CEL_K_PHOTON, n);
+  if (!merge_photon) {
+    if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
+    after_launch(c, CEL_K_PHOTON, n);
+  }
   // (in the masked modes the annihilation kernel precedes it on the main stream)
   if (cyl) { if (field) launch_chain(c, k_charged<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 1, TR>, pg, kBlock, s); }
   else { if (field) launch_chain(c, k_charged<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 0, TR>, pg, kBlock, s); }

@@ -116,6 +116,8 @@ struct Control {
   uint32_t ticket_fill, ticket_push;
   uint32_t n_logged;
   uint32_t vac_total;               // V before the fill of this iteration
+  unsigned long long n_init_fill;   // I after the fill of this iteration (= n_init until k_push adds S)
+  uint32_t iter_cur;                // k of the running iteration, a copy k_push may read while its block 0 bumps iter
   uint32_t part_charged;            // sort mode 3: charged initializers among the n_take popped in this iteration
   unsigned long long barrier;       // arrival counter of the persistent kernel's grid barrier (zeroed per launch)
 };

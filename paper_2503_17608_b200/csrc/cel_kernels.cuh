@@ -487,6 +487,8 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
   const unsigned long long Iafter = I - n_take;   // I -= min(V, I)
   ctl->vac_total = V;
   ctl->n_init = Iafter;
+  ctl->n_init_fill = Iafter;   // what k_push reads (it writes n_init itself)
+  ctl->iter_cur = ctl->iter;
   ctl->alive = alive;
   if (alive == 0 && Iafter == 0) {
     ctl->finished = 1;
@@ -524,6 +526,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   const unsigned long long I = ctl->n_init;
   if (finished) return;
   const TraceScope<K_INIT_FILL, TRACE> trace(D, iter);
+  if (threadIdx.x == 8) D.tile_sec[tile] = 0;   // consumed by the push of the previous iteration
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
   fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
@@ -600,9 +603,12 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   pdl_prologue();
   Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
-  const uint32_t finished = ctl->finished, iter = ctl->iter;
+  // No "last block" here: every block forms S itself, and block 0 alone updates the control block — it writes only fields
+  // that no block of this kernel reads (n_init and iter are read through the copies k_init_fill left: n_init_fill,
+  // iter_cur). The per-tile counters are zeroed by the next k_init_fill.
+  const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
   const int32_t error = ctl->error;
-  const unsigned long long I = ctl->n_init;
+  const unsigned long long I = ctl->n_init_fill;
   uint32_t cnt[kCountersPerThread];
   load_counters(D.tile_sec, D.n_tiles, cnt);
   if (finished) return;
@@ -610,17 +616,14 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   uint32_t prefix, S, tile_total;
   block_prefix_total_regs(cnt, tile, sm.scan, prefix, S, tile_total);
   const bool overflow = error != 0 || I + S > D.init_capacity;
-  push_tile(D, sm, tile, I, prefix, tile_total, overflow);
-  if (last_block_done(&ctl->ticket_push)) {
-    for (uint32_t i = threadIdx.x; i < D.n_tiles; i += kTileThreads) D.tile_sec[i] = 0;
-    if (threadIdx.x == 0) {
-      ctl->push_total = S;
-      if (I + S > D.init_capacity) ctl->error = -4;  // CEL_ERR_INIT_OVERFLOW (sticky)
-      else if (error == 0) ctl->n_init = I + S;
-      ctl->secondaries += S;
-      ctl->iter = iter + 1;
-    }
+  if (tile == 0 && threadIdx.x == 0) {
+    ctl->push_total = S;
+    if (I + S > D.init_capacity) ctl->error = -4;  // CEL_ERR_INIT_OVERFLOW (sticky)
+    else if (error == 0) ctl->n_init = I + S;
+    ctl->secondaries += S;
+    ctl->iter = iter + 1;
   }
+  push_tile(D, sm, tile, I, prefix, tile_total, overflow);
 }
 
 // ================================================================ S9-P: charged / neutral partition of the popped initializers

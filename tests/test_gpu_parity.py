@@ -252,11 +252,12 @@ def test_merged_discrete_kernel_identical(binding):
     kernels: same tallies, per-iteration counts and counters"""
     for w0 in (W.config2(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
         w0.sort_mode = 1
-        a, ca = run_gpu(binding, w0, persistent=0, merge_discrete=1)
         b, cb = run_gpu(binding, w0, persistent=0, merge_discrete=0)
-        assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), w0.name
-        assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
-        assert a["kernel_launches"] < b["kernel_launches"]
+        for md in (1, 2):   # 2: the photon kernel in the same launch as well (k_neutral)
+            a, ca = run_gpu(binding, w0, persistent=0, merge_discrete=md)
+            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, md)
+            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
+            assert a["kernel_launches"] < b["kernel_launches"]
 
 
 def test_fused_and_per_action_launches_identical(binding):
