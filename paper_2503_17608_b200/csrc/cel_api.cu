@@ -478,7 +478,8 @@ int enqueue_iteration_t(cel_ctx* c) {
     launch_chain(c, k_part_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_SCATTER, n);
   }
   launch_chain(c, k_init_fill<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_INIT_FILL, n);
-  if (D.sort_mode == CEL_SORT_BY_ACTION || D.sort_mode == CEL_SORT_BY_PARTICLE) { launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n); }
+  // (every sort mode: besides the index scatter of the sorted modes it closes the fill — vacancy counters, control block)
+  launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n);
   if (D.sort_mode == CEL_SORT_BY_ACTION && c->fused) {
     // one launch walks the chunks of every action's range (k_actions): the whole iteration is one PDL chain
     if (cyl) { if (field) launch_chain(c, k_actions<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 1, TR>, pg, kBlock, s); }
@@ -593,7 +594,8 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
   const uint64_t o_phist = align_up(o_hist + tiles * 32, 256);
   const uint64_t o_part = align_up(o_phist + tiles * 32, 256);
-  const uint64_t o_group = align_up(o_part + tiles * 4, 256);
+  const uint64_t o_filled = align_up(o_part + tiles * 4, 256);
+  const uint64_t o_group = align_up(o_filled + tiles * 4, 256);
   const uint64_t group_bytes = 2ull * kMaxGroups * 8 * sizeof(uint32_t);
   const uint64_t scratch_bytes = align_up(o_group + 2 * group_bytes, 256);
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
@@ -604,6 +606,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   D.tile_phist = (uint32_t*)((char*)c->scratch + o_phist);
   D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
   D.part_cnt = (uint32_t*)((char*)c->scratch + o_part);
+  D.tile_filled = (uint32_t*)((char*)c->scratch + o_filled);
   D.group_hist = (uint32_t*)((char*)c->scratch + o_group);
   D.group_phist = (uint32_t*)((char*)c->scratch + o_group + group_bytes);
   D.tally = (unsigned long long*)c->d_tally;

@@ -150,6 +150,7 @@ struct DeviceState {
   uint32_t* tile_phist;   // [n_tiles][8] per-tile particle histogram, 4 used (sort by particle)
   uint32_t* group_hist;   // [2][kMaxGroups][8] action counts per group of 32 tiles, double-buffered by iteration parity
   uint32_t* group_phist;  // [2][kMaxGroups][8] the same for the particle sort keys
+  uint32_t* tile_filled;  // [n_tiles] vacancies of the tile that k_init_fill filled in this iteration (k_scatter takes them off tile_vac)
   uint32_t* part_cnt;     // [n_tiles] sort mode 3: charged pops per tile-sized chunk of the popped segment
   // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
   // in / last warp out of every kernel of every iteration; nullptr = off

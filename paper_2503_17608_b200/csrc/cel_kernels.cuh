@@ -504,8 +504,7 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
 }
 
 // ================================================================ the bookkeeping kernels (one block per tile)
-// k_init_fill: P1 + the per-tile and per-group histograms; its last block takes the filled vacancies off tile_vac, sums
-// the group rows into the iteration's counts and updates offsets, ranges, counters and the log.
+// k_init_fill: P1 + the per-tile and per-group histograms.
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
@@ -534,65 +533,76 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   publish_tile_hist(D, sm, tile);
   const uint32_t parity = iter & 1u;
   publish_group_hist(D, sm, tile, parity);
-  if (!last_block_done(&ctl->ticket_fill)) return;
-  // ---- last block: thread t owns `per` consecutive tiles
-  const uint32_t per = (D.n_tiles + kTileThreads - 1) / kTileThreads;   // <= kMaxTiles / 256 = 8
-  const uint32_t t0 = threadIdx.x * per, t1 = min(D.n_tiles, t0 + per);
-  {  // vacancies left per tile
-    uint32_t v[kMaxTiles / kTileThreads];
-    uint32_t sum = 0;
-#pragma unroll
-    for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) { v[i] = (t0 + i < t1) ? D.tile_vac[t0 + i] : 0; sum += v[i]; }
-    uint32_t total;
-    uint32_t ex = block_excl_scan(sum, sm.scan, total);
-#pragma unroll
-    for (uint32_t i = 0; i < kMaxTiles / kTileThreads; ++i) {
-      if (t0 + i < t1) D.tile_vac[t0 + i] = v[i] - filled_by_plan(v[i], ex, plan);
-      ex += v[i];
-    }
-  }
-  // column sums of the group rows = the iteration's action counts (and sort-key counts)
-  __shared__ uint32_t act_part[2][8], key_part[2][8];
-  const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
-  const uint32_t n_groups = (D.n_tiles + kGroupTiles - 1) / kGroupTiles;
-  group_totals(group_rows(D.group_hist, parity), n_groups, act_part);
-  if (D.sort_mode == 2) group_totals(group_rows(D.group_phist, parity), n_groups, key_part);
-  __syncthreads();
+  // No "last block": the block leaves what it filled for k_reindex to take off tile_vac (other blocks of THIS kernel
+  // may still be reading the counters), and block 0 leaves the iteration's scalars in fields no fill block reads.
   if (threadIdx.x == 0) {
-    uint32_t act_total[8], key_total[8];
-    for (int k = 0; k < 8; ++k) { act_total[k] = act_part[0][k] + act_part[1][k]; key_total[k] = D.sort_mode == 2 ? key_part[0][k] + key_part[1][k] : act_total[k]; }
-    update_control_after_fill(D, act_total, key_total, n_keys, I, V, n_take);
+    D.tile_filled[tile] = filled_by_plan(tile_vacant, prefix, plan);
+    if (tile == 0) { ctl->vac_total = V; ctl->n_init_fill = I - n_take; ctl->iter_cur = iter; }
   }
 }
 
+// k_reindex (every sort mode): takes the filled vacancies off tile_vac; every block sums the <= 64 group rows into the
+// iteration's action / sort-key counts, hence the key offsets; block 0 writes them with ranges, counters and the log
+// to the control block (S11); in the sorted modes the block then scatters its tile's slot indices (P2).
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
-  const Control* ctl = D.ctl;
+  Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
   const uint32_t finished = ctl->finished, iter = ctl->iter;
-  const uint32_t tile_vacant = D.tile_vac[tile];
-  const uint32_t my_offset = threadIdx.x < 8 ? ctl->offsets[threadIdx.x] : 0u;
-  if (finished) return;
+  const uint32_t tile_vacant = D.tile_vac[tile] - D.tile_filled[tile];
+  const unsigned long long Iafter = ctl->n_init_fill;
+  const uint32_t V = ctl->vac_total;
+  if (finished) return;   // (block 0 may set it below while others start: they then skip work nobody needs any more)
   const TraceScope<K_SCATTER, TRACE> trace(D, iter);
-  {  // base[key] = offset[key] + (groups before the tile's group)[key] + (tiles of the group before the tile)[key]
+  if (threadIdx.x == 0) D.tile_vac[tile] = tile_vacant;
+  const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
+  {
     const uint32_t parity = iter & 1u;
-    const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5;
-    __shared__ uint32_t part[3][8];
-    if (warp < 3) {
-      uint32_t s8[8];
-      const uint32_t* grows = group_rows(D.sort_mode == 2 ? D.group_phist : D.group_hist, parity);
-      if (warp < 2) warp_sum_rows(grows + (size_t)warp * 32 * 8, g > warp * 32 ? min(32u, g - warp * 32) : 0u, s8);
-      else warp_sum_rows(sort_rows(D) + (size_t)g * kGroupTiles * 8, tile - g * kGroupTiles, s8);
-      if ((threadIdx.x & 31) == 0) {
+    const uint32_t n_groups = (D.n_tiles + kGroupTiles - 1) / kGroupTiles;
+    const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __shared__ uint32_t act_part[2][8], key_part[2][8], before[3][8], off_s[9];
+    if (warp < 2) {   // warp w sums the group rows [32 w, 32 w + 32): all of them (totals) and those before the tile's group
+      const uint32_t row = warp * 32 + lane;
+      const uint32_t* arows = group_rows(D.group_hist, parity);
+      const uint32_t* krows = D.sort_mode == 2 ? group_rows(D.group_phist, parity) : arows;
+      uint4 a0 = make_uint4(0, 0, 0, 0), a1 = a0, k0 = a0, k1 = a0;
+      if (row < n_groups) {
+        a0 = *reinterpret_cast<const uint4*>(arows + row * 8); a1 = *reinterpret_cast<const uint4*>(arows + row * 8 + 4);
+        if (D.sort_mode == 2) { k0 = *reinterpret_cast<const uint4*>(krows + row * 8); k1 = *reinterpret_cast<const uint4*>(krows + row * 8 + 4); }
+        else { k0 = a0; k1 = a1; }
+      }
+      const uint32_t av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
+      const uint32_t kv[8] = {k0.x, k0.y, k0.z, k0.w, k1.x, k1.y, k1.z, k1.w};
+      const bool bef = row < g;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) part[warp][k] = s8[k];
+      for (int k = 0; k < 8; ++k) {
+        const uint32_t ta = __reduce_add_sync(0xffffffffu, av[k]);
+        const uint32_t tk = __reduce_add_sync(0xffffffffu, kv[k]);
+        const uint32_t tb = __reduce_add_sync(0xffffffffu, bef ? kv[k] : 0u);
+        if (lane == 0) { act_part[warp][k] = ta; key_part[warp][k] = tk; before[warp][k] = tb; }
+      }
+    } else if (warp == 2) {   // the tile rows of the own group before the tile
+      uint32_t s8[8];
+      warp_sum_rows(sort_rows(D) + (size_t)g * kGroupTiles * 8, n_keys ? tile - g * kGroupTiles : 0u, s8);
+      if (lane == 0) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) before[2][k] = s8[k];
       }
     }
     __syncthreads();
-    if (threadIdx.x < 8) sm.base[threadIdx.x] = my_offset + part[0][threadIdx.x] + part[1][threadIdx.x] + part[2][threadIdx.x];
+    if (threadIdx.x == 0) {
+      uint32_t act_total[8], key_total[8];
+      for (int k = 0; k < 8; ++k) { act_total[k] = act_part[0][k] + act_part[1][k]; key_total[k] = key_part[0][k] + key_part[1][k]; }
+      uint32_t o = 0;
+      for (int k = 0; k < 8; ++k) { off_s[k] = o; if (k < n_keys) o += key_total[k]; }
+      if (tile == 0) update_control_after_fill(D, act_total, key_total, n_keys, Iafter, V, 0u);
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) sm.base[threadIdx.x] = off_s[threadIdx.x] + before[0][threadIdx.x] + before[1][threadIdx.x] + before[2][threadIdx.x];
   }
+  if (n_keys == 0) return;   // modes none / partition: no index array
   __syncthreads();
   scatter_tile(D, sm, tile, tile_vacant);
 }
