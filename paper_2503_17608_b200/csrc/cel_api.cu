@@ -513,7 +513,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     if (cyl) k_neutral<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_neutral<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
     after_launch(c, CEL_K_DISCRETE, n);
   } else if (by_action && c->merge_discrete) {
-    const int dg = pg < 2 * c->n_sm ? pg : 2 * c->n_sm;
+    const int dg = pg < c->n_sm ? pg : c->n_sm;   // one block per SM: the ranges are small, and a small grid launches faster
     k_discrete<TR><<<dg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_DISCRETE, n);
   } else {
     if (c->phys.enable_annihilation) { k_annihilation<TR><<<pg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_ANNIH, n); }
