@@ -147,8 +147,9 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * chain (default 1). persistent: the cooperative one-kernel form (default 0). fused: sorted by action, launch the
  * five action kernels as one grid that walks the chunks of every action's range; in the masked modes, one launch
  * with one thread per slot and the action switched on (default 0 = one launch per action; DESIGN.md section 10 has the
- * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). merge_discrete: sorted by action, photoelectric + pair + annihilation
- * in one launch (default 1). trace: see cel_trace. */
+ * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). merge_discrete: photoelectric + pair + annihilation in one launch (default 1:
+ * sorted by action over their three ranges, unsorted / partition as one masked pass before the move kernels; 2: sorted
+ * by action with the photon kernel in the same launch; 0: one launch per action). trace: see cel_trace. */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a

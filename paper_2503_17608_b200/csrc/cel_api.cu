@@ -497,6 +497,21 @@ int enqueue_iteration_t(cel_ctx* c) {
   }
   const bool fork = c->concurrent && !c->profile;
   const bool by_action = D.sort_mode == CEL_SORT_BY_ACTION;
+  if ((D.sort_mode == CEL_SORT_NONE || D.sort_mode == CEL_SORT_PARTITION) && c->merge_discrete) {
+    // unsorted / partition: the three pure interactions in one pass on the main stream, then photon beside charged
+    // (measured +2..5 %; by particle the two chains below are as fast or faster)
+    launch_chain(c, k_discrete_masked<TR>, pg, kBlock, s); after_launch(c, CEL_K_DISCRETE, n);
+    cudaStream_t sp = s;
+    if (fork) { cudaEventRecord(c->ev_fork, s); cudaStreamWaitEvent(c->side[0], c->ev_fork, 0); sp = c->side[0]; }
+    if (cyl) k_photon<1, TR><<<pg, kBlock, 0, sp>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, sp>>>(D);
+    after_launch(c, CEL_K_PHOTON, n);
+    if (cyl) { if (field) k_charged<true, 1, TR><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 1, TR><<<pg, kBlock, 0, s>>>(D); }
+    else { if (field) k_charged<true, 0, TR><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0, TR><<<pg, kBlock, 0, s>>>(D); }
+    after_launch(c, CEL_K_CHARGED, n);
+    if (fork) { cudaEventRecord(c->ev_join[0], c->side[0]); cudaStreamWaitEvent(s, c->ev_join[0], 0); }
+    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    return n;
+  }
   // sorted by action: photon, annihilation, photoelectric, pair on one branch each (their ranges are disjoint and fixed);
   // masked modes: {photoelectric -> pair -> photon} on one branch beside {annihilation -> charged} on the main stream
   cudaStream_t s_photon = s, s_annih = s, s_pe = s, s_pair = s;

@@ -511,6 +511,31 @@ __global__ void __launch_bounds__(kBlock) k_discrete(DeviceState D) {
   }
 }
 
+// The masked modes' form: one pass over the kernel's index range, the key byte picks the three pure interactions. It
+// runs BEFORE the two move kernels (a move kernel rewrites key bytes into PE / PAIR / ANNIH, which must not be applied
+// in the same iteration), replacing the chains {annihilation -> charged} and {photoelectric -> pair -> photon}.
+template <bool TRACE>
+__global__ void __launch_bounds__(kBlock) k_discrete_masked(DeviceState D) {
+  pdl_prologue();
+  const Control* ctl = D.ctl;
+  const uint32_t finished_ = ctl->finished;
+  const uint32_t re = D.sort_mode == 2 ? ctl->offsets[3] : D.N;   // by particle: the non-vacant part of the index array
+  const uint32_t k_iter = ctl->iter;
+  if (finished_) return;
+  const TraceScope<K_DISCRETE, TRACE> trace(D, k_iter);
+  for (uint32_t tid = blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x) {
+    const uint32_t slot = slot_of(D, tid);
+    const int ak = D.akey[slot] & 0xf;
+    if (ak != A_PE && ak != A_PAIR && ak != A_ANNIH) continue;
+    const RecB b = load_b(D.stB + slot);
+    const RecA a = load_a(D.stA + slot);
+    const int act = meta_action(b.meta);
+    if (act == A_PE) do_photoelectric(D, slot, a, b);
+    else if (act == A_PAIR) do_pair(D, slot, k_iter, a, b);
+    else if (act == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
+  }
+}
+
 // The same with the photon kernel in the launch as well (option merge_discrete = 2): photon chunks first (the heavy
 // part), then the three pure interactions. Two action launches per iteration: this one beside k_charged. Runs at the
 // photon kernel's register count, which the three small actions do not mind.

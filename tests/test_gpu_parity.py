@@ -260,6 +260,19 @@ def test_merged_discrete_kernel_identical(binding):
             assert a["kernel_launches"] < b["kernel_launches"]
 
 
+def test_merged_discrete_masked_identical(binding):
+    """unsorted / partition: photoelectric + pair + annihilation in one masked pass before the move kernels
+    (k_discrete_masked, the default) and as the two kernel chains: same tallies, counts and counters"""
+    for w0 in (W.config3(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
+        for mode in (0, 3):
+            w0.sort_mode = mode
+            a, ca = run_gpu(binding, w0, persistent=0, merge_discrete=1)
+            b, cb = run_gpu(binding, w0, persistent=0, merge_discrete=0)
+            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
+            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
+            assert a["kernel_launches"] < b["kernel_launches"]
+
+
 def test_fused_and_per_action_launches_identical(binding):
     """the one-launch forms (sorted by action: k_actions walks the chunks of every action's range; masked modes:
     k_actions_masked, one thread per slot with the action switched on) and the launch-per-action form give the same
