@@ -593,7 +593,7 @@ __global__ void __launch_bounds__(kBlock) k_neutral(DeviceState D) {
 // iteration loses four launches, the fork / join of the side streams, and the tail in which the small kernels queued
 // behind the blocks of the big ones (profiles/: timeline). Results are bit-identical to the kernel-per-action form.
 template <bool FIELD, int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock) k_actions(DeviceState D) {
+__global__ void __launch_bounds__(kBlock, FIELD ? 2 : 4) k_actions(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
   if (ctl->finished) return;
