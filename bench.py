@@ -336,7 +336,9 @@ def run_cuda(args):
                          "alg_bytes": alg[name], "gbs": round(gbs, 2), "frac": round(gbs / peak, 4)}
     dominant = max(kernels, key=lambda k: kernels[k]["ms"])
     dk = kernels[dominant]
-    traffic, traffic_it = load_profile_traffic(dominant)
+    # the committed ncu capture is of the default workload (config 2, by action, 2^20 slots): no traffic figure for others
+    is_default = args.workload == "config2" and w.sort_mode == 1 and not args.events and not args.slots and not args.max_substeps
+    traffic, traffic_it = load_profile_traffic(dominant) if is_default else (None, None)
     alg_at_it = None
     if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "actions", "discrete"):
         alg_at_it = algorithmic_bytes(counts[traffic_it:traffic_it + 1], w.n_slots, w.sort_mode, 0, 0)[dominant]
