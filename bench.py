@@ -181,7 +181,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     sec = float(n_secondaries)
     out = {
         "init_fill": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES,   # key bytes + (read init, write slot)
-        "scatter": it * n * (1 + INDEX_BYTES),
+        "scatter": it * n * 1 + (it * n - c[7]) * idx,                      # key bytes + one index per non-vacant slot
         "annihilation": c[6] * (rw + 2 * STATE_BYTES),
         "photoelectric": c[0] * (rw + STATE_BYTES),
         "pair": c[1] * (rw + 2 * STATE_BYTES),
