@@ -1,8 +1,13 @@
 // cel_kernels.cuh — the bookkeeping kernels of one step iteration (docs/PHYSICS_SPEC.md S1):
 //   P1 init + P2 histogram: k_init_fill   (scan-based vacancy filling, S9; per-tile sort-key histogram, S2)
-//   P2 reindex:             k_scatter     (stable counting sort of slot indices, S2)
+//   P2 reindex:             k_scatter     (closes the fill: vacancy counters, action counts, offsets, control block;
+//                                          then the stable counting sort of slot indices, S2)
 //   P5 push:                k_push        (scan-ordered secondary push, S9)
+//   S9-P (sort mode 3):     k_part_count, k_part_scatter (charged / neutral partition of the popped initializers)
 // (P3/P4, the action kernels and the scoring, are in cel_physics.cuh.)
+// No kernel has a "last block" phase: what one block would have to do after all the others (scans over tiles, the
+// control block) is either done redundantly by every block from small two-level counters, or left to the blocks of
+// the next kernel.
 // The action kernels keep two per-tile counters up to date with integer atomics — vacancies created and secondaries
 // staged — so neither scan needs a counting pass: a block reduces the counters of the tiles before it to get its
 // exclusive prefix, skips its tile when there is nothing to fill / push, and otherwise scans the tile's dense key
@@ -533,7 +538,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   publish_tile_hist(D, sm, tile);
   const uint32_t parity = iter & 1u;
   publish_group_hist(D, sm, tile, parity);
-  // No "last block": the block leaves what it filled for k_reindex to take off tile_vac (other blocks of THIS kernel
+  // No "last block": the block leaves what it filled for k_scatter to take off tile_vac (other blocks of THIS kernel
   // may still be reading the counters), and block 0 leaves the iteration's scalars in fields no fill block reads.
   if (threadIdx.x == 0) {
     D.tile_filled[tile] = filled_by_plan(tile_vacant, prefix, plan);
@@ -541,7 +546,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   }
 }
 
-// k_reindex (every sort mode): takes the filled vacancies off tile_vac; every block sums the <= 64 group rows into the
+// k_scatter (every sort mode; "reindex + close the fill"): takes the filled vacancies off tile_vac; every block sums the <= 64 group rows into the
 // iteration's action / sort-key counts, hence the key offsets; block 0 writes them with ranges, counters and the log
 // to the control block (S11); in the sorted modes the block then scatters its tile's slot indices (P2).
 template <bool TRACE>
