@@ -187,7 +187,10 @@ Tiling make_tiling(uint64_t N) {
   const uint64_t subs = (N + kSub - 1) / kSub;
   uint32_t spt = 1, shift = 10;
   static_assert(kSub == 1024, "tile_shift assumes 1024-slot sub-tiles");
-  while ((subs + spt - 1) / spt > (uint64_t)kMaxTiles) { spt *= 2; shift += 1; }
+  // at most 2048 tiles up to 2^22 slots, kMaxTiles = 4096 beyond (measured: more, smaller tiles pay only when a block
+  // would otherwise walk 8 sub-tiles; at 2^22 slots 4096 blocks per bookkeeping kernel raise the per-iteration floor)
+  const uint64_t max_tiles = N > (1ull << 22) ? (uint64_t)kMaxTiles : 2048ull;
+  while ((subs + spt - 1) / spt > max_tiles) { spt *= 2; shift += 1; }
   Tiling t;
   t.subs_per_tile = spt; t.tile_shift = shift;
   t.n_tiles = (uint32_t)((N + ((uint64_t)1 << shift) - 1) >> shift);
@@ -477,7 +480,9 @@ int enqueue_iteration_t(cel_ctx* c) {
     launch_chain(c, k_part_count<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_COUNT, n);
     launch_chain(c, k_part_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_SCATTER, n);
   }
-  launch_chain(c, k_init_fill<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_INIT_FILL, n);
+  const bool many_tiles = D.n_tiles > 2048u;   // 16 instead of 8 tile counters per thread in the block prefix
+  if (many_tiles) launch_chain(c, k_init_fill<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_init_fill<TR, 8>, tg, kTileThreads, s);
+  after_launch(c, CEL_K_INIT_FILL, n);
   // (every sort mode: besides the index scatter of the sorted modes it closes the fill — vacancy counters, control block)
   launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n);
   if (D.sort_mode == CEL_SORT_BY_ACTION && c->fused) {
@@ -485,14 +490,14 @@ int enqueue_iteration_t(cel_ctx* c) {
     if (cyl) { if (field) launch_chain(c, k_actions<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 1, TR>, pg, kBlock, s); }
     else { if (field) launch_chain(c, k_actions<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 0, TR>, pg, kBlock, s); }
     after_launch(c, CEL_K_ACTIONS, n);
-    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
     return n;
   }
   if (c->fused) {   // masked modes: one launch, one thread per slot, the action switched on (k_actions_masked)
     if (cyl) { if (field) launch_chain(c, k_actions_masked<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 1, TR>, pg, kBlock, s); }
     else { if (field) launch_chain(c, k_actions_masked<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 0, TR>, pg, kBlock, s); }
     after_launch(c, CEL_K_ACTIONS, n);
-    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
     return n;
   }
   const bool fork = c->concurrent && !c->profile;
@@ -509,7 +514,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     else { if (field) k_charged<true, 0, TR><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0, TR><<<pg, kBlock, 0, s>>>(D); }
     after_launch(c, CEL_K_CHARGED, n);
     if (fork) { cudaEventRecord(c->ev_join[0], c->side[0]); cudaStreamWaitEvent(s, c->ev_join[0], 0); }
-    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
     return n;
   }
   // sorted by action: photon, annihilation, photoelectric, pair on one branch each (their ranges are disjoint and fixed);
@@ -547,7 +552,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     cudaEventRecord(c->ev_join[i], c->side[i]);
     cudaStreamWaitEvent(s, c->ev_join[i], 0);
   }
-  launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+  if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
   return n;
 }
 int enqueue_iteration(cel_ctx* c) { return c->trace_iters > 0 ? enqueue_iteration_t<true>(c) : enqueue_iteration_t<false>(c); }

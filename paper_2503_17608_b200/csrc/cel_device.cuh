@@ -97,7 +97,7 @@ struct Params {
 constexpr int kTileThreads = 256;
 constexpr int kKeysPerThread = 4;
 constexpr int kSub = kTileThreads * kKeysPerThread;  // 1024 slots per sub-tile
-constexpr int kMaxTiles = 2048;
+constexpr int kMaxTiles = 4096;
 
 // index ranges of the action kernels in the sorted index array (S2)
 enum KernelRange : int { R_PE = 0, R_PAIR, R_ANNIH, R_PHOTON, R_CHARGED, R_COUNT };

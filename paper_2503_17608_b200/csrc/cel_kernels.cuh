@@ -107,16 +107,19 @@ __device__ __forceinline__ void block_prefix_total(const uint32_t* a, uint32_t n
 // The same with the counters already in registers: load_counters issues every load of the kernel's prologue back to
 // back (control block, counters) BEFORE the first use, so the prologue costs one L2 round trip instead of one per
 // dependent step (in-order issue stalls at the first use). Also returns a[tile].
-constexpr int kCountersPerThread = kMaxTiles / kTileThreads;   // 8
-__device__ __forceinline__ void load_counters(const uint32_t* a, uint32_t n, uint32_t (&v)[kCountersPerThread]) {
+// (CPT counters per thread: 8 up to 2048 tiles, 16 above — two instantiations of the kernels that use it, so that the
+// common sizes keep their register count)
+template <int CPT>
+__device__ __forceinline__ void load_counters(const uint32_t* a, uint32_t n, uint32_t (&v)[CPT]) {
 #pragma unroll
-  for (int i = 0; i < kCountersPerThread; ++i) { const uint32_t idx = threadIdx.x + i * kTileThreads; v[i] = idx < n ? a[idx] : 0u; }
+  for (int i = 0; i < CPT; ++i) { const uint32_t idx = threadIdx.x + i * kTileThreads; v[i] = idx < n ? a[idx] : 0u; }
 }
-__device__ __forceinline__ void block_prefix_total_regs(const uint32_t (&v)[kCountersPerThread], uint32_t tile, uint32_t* smem /* 19 words */,
+template <int CPT>
+__device__ __forceinline__ void block_prefix_total_regs(const uint32_t (&v)[CPT], uint32_t tile, uint32_t* smem /* 19 words */,
                                                         uint32_t& prefix, uint32_t& total, uint32_t& own) {
   uint32_t p = 0, t = 0;
 #pragma unroll
-  for (int i = 0; i < kCountersPerThread; ++i) {
+  for (int i = 0; i < CPT; ++i) {
     const uint32_t idx = threadIdx.x + i * kTileThreads;
     t += v[i];
     if (idx < tile) p += v[i];
@@ -127,28 +130,13 @@ __device__ __forceinline__ void block_prefix_total_regs(const uint32_t (&v)[kCou
   __syncthreads();
   if (lane == 0) { smem[warp] = p; smem[9 + warp] = t; }
 #pragma unroll
-  for (int i = 0; i < kCountersPerThread; ++i) if (threadIdx.x + i * kTileThreads == tile) smem[18] = v[i];
+  for (int i = 0; i < CPT; ++i) if (threadIdx.x + i * kTileThreads == tile) smem[18] = v[i];
   __syncthreads();
   p = 0; t = 0;
 #pragma unroll
   for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
   prefix = p; total = t; own = smem[18];
 }
-// "last block done" ticket: true in exactly one block, after every other block's global writes are visible
-__device__ __forceinline__ bool last_block_done(uint32_t* ticket) {
-  __shared__ bool is_last;
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    uint32_t t = atomicAdd(ticket, 1u);
-    is_last = (t == gridDim.x - 1);
-    if (is_last) *ticket = 0;
-  }
-  __syncthreads();
-  if (is_last) __threadfence();
-  return is_last;
-}
-
 __device__ __forceinline__ int sort_key_of(int sort_mode, uint32_t key) {
   const int a = key & 0xf;
   if (sort_mode == 1) return a;
@@ -280,12 +268,12 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
 // Two-level histograms. Besides its own row tile_hist[tile][8], every fill block adds its counts into the row of its
 // GROUP of kGroupTiles tiles (integer atomics on 8 x n_groups addresses, double-buffered by the parity of the iteration:
 // the blocks of iteration k also zero the rows that iteration k+1 will add into). Column totals are then the sum of
-// <= 64 group rows, and the base of a tile in the counting sort is (groups before its group) + (tiles of its group
+// <= 128 group rows, and the base of a tile in the counting sort is (groups before its group) + (tiles of its group
 // before it): 2 KB read by each scatter block, 2 KB by the one block that updates the control block — instead of one
 // block scanning all 32 KB of rows in place, which was 4.4 of the 12 us of an almost empty k_init_fill (one SM pulls
 // ~64 B per clock from L2; profiles/).
 constexpr int kGroupTiles = 32;
-constexpr int kMaxGroups = kMaxTiles / kGroupTiles;   // 64
+constexpr int kMaxGroups = kMaxTiles / kGroupTiles;   // 128
 __device__ __forceinline__ uint32_t* group_rows(uint32_t* base, uint32_t parity) { return base + (size_t)parity * kMaxGroups * 8; }
 // after fill_tile + __syncthreads: publish the tile's action histogram and (sort by particle) its sort-key histogram.
 // The iteration's action counts are the column sums of tile_hist (no same-address atomics from a thousand blocks).
@@ -311,42 +299,6 @@ __device__ __forceinline__ void publish_group_hist(const DeviceState& D, BookSme
 // the rows the scatter takes its per-tile bases from: the action histogram (sort by action) or the particle histogram
 __device__ __forceinline__ uint32_t* sort_rows(const DeviceState& D) { return D.sort_mode == 2 ? D.tile_phist : D.tile_hist; }
 
-// in-place exclusive scan over the tiles of the 8 columns of rows[n_tiles][8] by one block, in one pass: thread t owns
-// the tiles [t0, t1); the column totals go to total[8] (shared). write_back = false only computes the totals.
-__device__ __forceinline__ void scan_tile_rows(uint32_t* rows, uint32_t t0, uint32_t t1, bool write_back,
-                                               uint32_t (*warp_tot)[8] /* shared [8][8] */, uint32_t* total /* shared 8 */) {
-  uint32_t acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-  for (uint32_t t = t0; t < t1; ++t) {
-    const uint4 a = *reinterpret_cast<const uint4*>(rows + t * 8), b = *reinterpret_cast<const uint4*>(rows + t * 8 + 4);
-    acc[0] += a.x; acc[1] += a.y; acc[2] += a.z; acc[3] += a.w; acc[4] += b.x; acc[5] += b.y; acc[6] += b.z; acc[7] += b.w;
-  }
-  uint32_t ex[8];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    const uint32_t incl = warp_incl_scan(acc[k]);
-    ex[k] = incl - acc[k];
-    if (lane == 31) warp_tot[warp][k] = incl;
-  }
-  __syncthreads();
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    uint32_t before = 0, all = 0;
-#pragma unroll
-    for (int w = 0; w < kTileThreads / 32; ++w) { const uint32_t v = warp_tot[w][k]; all += v; if (w < warp) before += v; }
-    ex[k] += before;
-    if (threadIdx.x == 0) total[k] = all;
-  }
-  if (write_back) {
-    for (uint32_t t = t0; t < t1; ++t) {
-      uint4* pa = reinterpret_cast<uint4*>(rows + t * 8); uint4* pb = reinterpret_cast<uint4*>(rows + t * 8 + 4);
-      const uint4 a = *pa, b = *pb;
-      *pa = make_uint4(ex[0], ex[1], ex[2], ex[3]); *pb = make_uint4(ex[4], ex[5], ex[6], ex[7]);
-      ex[0] += a.x; ex[1] += a.y; ex[2] += a.z; ex[3] += a.w; ex[4] += b.x; ex[5] += b.y; ex[6] += b.z; ex[7] += b.w;
-    }
-  }
-  __syncthreads();
-}
 // sum over the rows r < n_rows (n_rows <= 32) of rows[r][0..8) by one warp; every lane gets the 8 column sums
 __device__ __forceinline__ void warp_sum_rows(const uint32_t* rows, uint32_t n_rows, uint32_t* out8) {
   const uint32_t lane = threadIdx.x & 31;
@@ -357,20 +309,6 @@ __device__ __forceinline__ void warp_sum_rows(const uint32_t* rows, uint32_t n_r
   out8[4] = __reduce_add_sync(0xffffffffu, b.x); out8[5] = __reduce_add_sync(0xffffffffu, b.y);
   out8[6] = __reduce_add_sync(0xffffffffu, b.z); out8[7] = __reduce_add_sync(0xffffffffu, b.w);
 }
-// column totals of all groups (n_groups <= 64) into total[8] (shared) by warps 0 and 1; the caller synchronises after
-__device__ __forceinline__ void group_totals(const uint32_t* grows, uint32_t n_groups, uint32_t (*part)[8] /* shared [2][8] */) {
-  const uint32_t warp = threadIdx.x >> 5;
-  if (warp < 2) {
-    uint32_t s8[8];
-    const uint32_t first = warp * 32;
-    warp_sum_rows(grows + (size_t)first * 8, n_groups > first ? min(32u, n_groups - first) : 0u, s8);
-    if ((threadIdx.x & 31) == 0) {
-#pragma unroll
-      for (int k = 0; k < 8; ++k) part[warp][k] = s8[k];
-    }
-  }
-}
-
 // vacancies of a tile that the fill of this iteration takes: min(v, max(0, n_take - (vacancies before the tile)))
 __device__ __forceinline__ uint32_t filled_in_tile(uint32_t v, uint32_t prefix, uint32_t n_take) {
   return min(v, n_take > prefix ? n_take - prefix : 0u);
@@ -510,7 +448,7 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
 
 // ================================================================ the bookkeeping kernels (one block per tile)
 // k_init_fill: P1 + the per-tile and per-group histograms.
-template <bool TRACE>
+template <bool TRACE, int CPT>
 __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   __shared__ BookSmem sm;
   Control* ctl = D.ctl;
@@ -520,11 +458,11 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   // plist): the vacancy counters and `finished` were last written by the action kernels / the previous k_init_fill,
   // which had completed before that kernel let this one start. The vacancy prefix so overlaps the push.
   const uint32_t finished = ctl->finished;
-  uint32_t cnt[kCountersPerThread];
-  load_counters(D.tile_vac, D.n_tiles, cnt);
+  uint32_t cnt[CPT];
+  load_counters<CPT>(D.tile_vac, D.n_tiles, cnt);
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
   uint32_t prefix, V, tile_vacant;
-  block_prefix_total_regs(cnt, tile, sm.scan, prefix, V, tile_vacant);   // (its barriers also publish sm.hist / sm.act)
+  block_prefix_total_regs<CPT>(cnt, tile, sm.scan, prefix, V, tile_vacant);   // (its barriers also publish sm.hist / sm.act)
   pdl_prologue();
   const uint32_t iter = ctl->iter, n_charged = ctl->part_charged;
   const unsigned long long I = ctl->n_init;
@@ -546,7 +484,7 @@ __global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
   }
 }
 
-// k_scatter (every sort mode; "reindex + close the fill"): takes the filled vacancies off tile_vac; every block sums the <= 64 group rows into the
+// k_scatter (every sort mode; "reindex + close the fill"): takes the filled vacancies off tile_vac; every block sums the <= 128 group rows into the
 // iteration's action / sort-key counts, hence the key offsets; block 0 writes them with ranges, counters and the log
 // to the control block (S11); in the sorted modes the block then scatters its tile's slot indices (P2).
 template <bool TRACE>
@@ -567,8 +505,9 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
     const uint32_t parity = iter & 1u;
     const uint32_t n_groups = (D.n_tiles + kGroupTiles - 1) / kGroupTiles;
     const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    __shared__ uint32_t act_part[2][8], key_part[2][8], before[3][8], off_s[9];
-    if (warp < 2) {   // warp w sums the group rows [32 w, 32 w + 32): all of them (totals) and those before the tile's group
+    constexpr int kGroupWarps = kMaxGroups / 32;   // 4
+    __shared__ uint32_t act_part[kGroupWarps][8], key_part[kGroupWarps][8], before[kGroupWarps + 1][8], off_s[9];
+    if (warp < (uint32_t)kGroupWarps) {   // warp w sums the group rows [32 w, 32 w + 32): all of them (totals) and those before the tile's group
       const uint32_t row = warp * 32 + lane;
       const uint32_t* arows = group_rows(D.group_hist, parity);
       const uint32_t* krows = D.sort_mode == 2 ? group_rows(D.group_phist, parity) : arows;
@@ -588,31 +527,38 @@ __global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
         const uint32_t tb = __reduce_add_sync(0xffffffffu, bef ? kv[k] : 0u);
         if (lane == 0) { act_part[warp][k] = ta; key_part[warp][k] = tk; before[warp][k] = tb; }
       }
-    } else if (warp == 2) {   // the tile rows of the own group before the tile
+    } else if (warp == (uint32_t)kGroupWarps) {   // the tile rows of the own group before the tile
       uint32_t s8[8];
       warp_sum_rows(sort_rows(D) + (size_t)g * kGroupTiles * 8, n_keys ? tile - g * kGroupTiles : 0u, s8);
       if (lane == 0) {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) before[2][k] = s8[k];
+        for (int k = 0; k < 8; ++k) before[kGroupWarps][k] = s8[k];
       }
     }
     __syncthreads();
     if (threadIdx.x == 0) {
       uint32_t act_total[8], key_total[8];
-      for (int k = 0; k < 8; ++k) { act_total[k] = act_part[0][k] + act_part[1][k]; key_total[k] = key_part[0][k] + key_part[1][k]; }
+      for (int k = 0; k < 8; ++k) {
+        act_total[k] = 0; key_total[k] = 0;
+        for (int w = 0; w < kGroupWarps; ++w) { act_total[k] += act_part[w][k]; key_total[k] += key_part[w][k]; }
+      }
       uint32_t o = 0;
       for (int k = 0; k < 8; ++k) { off_s[k] = o; if (k < n_keys) o += key_total[k]; }
       if (tile == 0) update_control_after_fill(D, act_total, key_total, n_keys, Iafter, V, 0u);
     }
     __syncthreads();
-    if (threadIdx.x < 8) sm.base[threadIdx.x] = off_s[threadIdx.x] + before[0][threadIdx.x] + before[1][threadIdx.x] + before[2][threadIdx.x];
+    if (threadIdx.x < 8) {
+      uint32_t b = off_s[threadIdx.x];
+      for (int w = 0; w <= kGroupWarps; ++w) b += before[w][threadIdx.x];
+      sm.base[threadIdx.x] = b;
+    }
   }
   if (n_keys == 0) return;   // modes none / partition: no index array
   __syncthreads();
   scatter_tile(D, sm, tile, tile_vacant);
 }
 
-template <bool TRACE>
+template <bool TRACE, int CPT>
 __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
@@ -624,12 +570,12 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
   const int32_t error = ctl->error;
   const unsigned long long I = ctl->n_init_fill;
-  uint32_t cnt[kCountersPerThread];
-  load_counters(D.tile_sec, D.n_tiles, cnt);
+  uint32_t cnt[CPT];
+  load_counters<CPT>(D.tile_sec, D.n_tiles, cnt);
   if (finished) return;
   const TraceScope<K_PUSH, TRACE> trace(D, iter);
   uint32_t prefix, S, tile_total;
-  block_prefix_total_regs(cnt, tile, sm.scan, prefix, S, tile_total);
+  block_prefix_total_regs<CPT>(cnt, tile, sm.scan, prefix, S, tile_total);
   const bool overflow = error != 0 || I + S > D.init_capacity;
   if (tile == 0 && threadIdx.x == 0) {
     ctl->push_total = S;

@@ -76,3 +76,18 @@ def test_partition_full_size(binding):
     o.transport(wo.primaries, wo.n_events)
     z = three_sigma(view["fixed"].astype(np.float64) * 2.0 ** -36, o.tallies())
     assert z.max() < 4.0 and (z > 3.0).mean() <= 0.02 + 1.0 / len(z)
+
+
+def test_more_than_2048_tiles(binding):
+    """above 2^22 slots the bookkeeping uses up to 4096 tiles (16 tile counters per thread in the block prefix, four
+    warps of group rows): a ragged slot count there, in lockstep with the oracle and bit-identical across sort modes"""
+    n_slots = (1 << 22) + 12345
+    w = W.config3(n_events=60, n_slots=n_slots, energy=3000.0, seed=9)
+    w.physics["init_capacity"] = 1 << 22
+    assert lockstep(binding, w, 4, must_match=3) >= 3
+    ref, ref_counts = run_gpu(binding, w)
+    whole_run_properties(ref, ref_counts, w)
+    for mode in (0, 2):
+        w.sort_mode = mode
+        v, c = run_gpu(binding, w)
+        assert np.array_equal(v["fixed"], ref["fixed"]) and np.array_equal(c, ref_counts), mode
