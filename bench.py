@@ -194,8 +194,6 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     out["part_scatter"] = float(n_initialised) * (8 + INDEX_BYTES)
     if sort_mode == 3:
         out["init_fill"] += float(n_initialised) * INDEX_BYTES
-    # sorted by action the five action kernels are one launch (k_actions): the same bytes, summed
-    out["actions"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair", "photon", "charged"))
     out["discrete"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair"))
     return out
 
@@ -340,7 +338,7 @@ def run_cuda(args):
     is_default = args.workload == "config2" and w.sort_mode == 1 and not args.events and not args.slots and not args.max_substeps
     traffic, traffic_it = load_profile_traffic(dominant) if is_default else (None, None)
     alg_at_it = None
-    if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "actions", "discrete"):
+    if traffic_it is not None and traffic_it < len(counts) and dominant in ("annihilation", "photoelectric", "pair", "photon", "charged", "discrete"):
         alg_at_it = algorithmic_bytes(counts[traffic_it:traffic_it + 1], w.n_slots, w.sort_mode, 0, 0)[dominant]
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": dk["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": dk["frac"], "traffic": traffic, "traffic_iteration": traffic_it,

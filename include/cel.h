@@ -126,7 +126,6 @@ const char* cel_last_cuda_error(cel_ctx*);
  * P3i: ANNIH, PE, PAIR; P3i+P3m: PHOTON (Compton, then the photon move), CHARGED (bremsstrahlung, then the charged move
  * with energy loss and MSC); P4 (scoring) happens inside the action kernels; P5: PUSH. */
 enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
-       CEL_K_ACTIONS /* the five action kernels in one launch (sort by action, option fused) */,
        CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
        CEL_K_DISCRETE /* photoelectric + pair + annihilation in one launch (sort by action, option merge_discrete) */,
        CEL_KERNEL_COUNT };
@@ -144,12 +143,10 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * per batch, so that cel_kernel_times can report per-kernel device time (a measurement mode: results are identical,
  * the run is slower). concurrent: 1 (default) = the independent action kernels of an iteration run as parallel
  * branches of the iteration graph; 0 = one after the other. pdl: programmatic dependent launch along the main
- * chain (default 1). persistent: the cooperative one-kernel form (default 0). fused: sorted by action, launch the
- * five action kernels as one grid that walks the chunks of every action's range; in the masked modes, one launch
- * with one thread per slot and the action switched on (default 0 = one launch per action; DESIGN.md section 10 has the
- * measurements: the one-launch form only pays together with CEL_SORT_PARTITION). merge_discrete: photoelectric + pair + annihilation in one launch (default 1:
- * sorted by action over their three ranges, unsorted / partition as one masked pass before the move kernels; 2: sorted
- * by action with the photon kernel in the same launch; 0: one launch per action). trace: see cel_trace. */
+ * chain (default 1). merge_discrete: photoelectric + pair + annihilation in one launch (default 1: sorted by action
+ * over their three ranges, unsorted / partition as one masked pass before the move kernels; 0: one launch per action).
+ * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
+ * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a

@@ -4,7 +4,6 @@
 #include "../../include/cel.h"
 #include "cel_kernels.cuh"
 #include "cel_physics.cuh"
-#include "cel_persistent.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -54,7 +53,6 @@ struct cel_ctx {
   cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
-  int fused = 0;   // sort by action: all action kernels in one launch (k_actions); measured equal (no field) to 6 % slower (field)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
   Control* h_status = nullptr;      // pinned, kStatusSlots entries
@@ -64,9 +62,6 @@ struct cel_ctx {
   int trace_iters = 0; int trace_ends = 1; void* d_trace = nullptr;   // option "trace": device-side timeline of the first trace_iters iterations
   DeviceState graph_D{}; int graph_cfg[6] = {-1, -1, -1, -1, -1, -1};   // what the captured graph has baked in (arguments, options)
   int use_graph = 1; int batch = 16; int64_t max_iterations = 1ll << 22;
-  int persistent = 0; int persist_batch = 64;   // one cooperative kernel runs up to persist_batch iterations
-  int persist_grid = 0;                         // co-resident blocks of k_persistent (0 = not available)
-  const void* persist_fn = nullptr;
   int n_sm = 148;
   bool ran = false; int run_error = 0;
   uint64_t launches = 0; int kernels_per_iteration = 0;
@@ -82,8 +77,6 @@ struct cel_ctx {
 };
 
 namespace {
-
-void setup_persistent(cel_ctx* c);   // defined with the host loop below
 
 #define CEL_CUDA(ctx, call)                                                        \
   do {                                                                             \
@@ -335,7 +328,6 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   const Tiling tl = make_tiling(n_slots);
   D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
   D.sort_mode = sort_mode;
-  setup_persistent(c);
   D.init_capacity = default_capacity(n_slots, ph->init_capacity);
 
   if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);
@@ -402,13 +394,10 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "batch")) { if (v < 1 || v > 4096) return CEL_ERR_INVALID_ARG; c->batch = (int)v; }
   else if (!std::strcmp(name, "profile")) c->profile = v ? 1 : 0;
   else if (!std::strcmp(name, "concurrent")) c->concurrent = v ? 1 : 0;
-  else if (!std::strcmp(name, "persistent")) c->persistent = v ? 1 : 0;
   else if (!std::strcmp(name, "pdl")) c->pdl = v ? 1 : 0;
-  else if (!std::strcmp(name, "fused")) c->fused = v ? 1 : 0;
-  else if (!std::strcmp(name, "merge_discrete")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->merge_discrete = (int)v; }
+  else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
-  else if (!std::strcmp(name, "persist_batch")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->persist_batch = (int)v; }
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
   return CEL_OK;
@@ -440,7 +429,7 @@ int physics_grid(const cel_ctx* c) {
 }
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
-    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push", "actions",
+    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push",
     "part_count", "part_scatter", "discrete"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
@@ -485,21 +474,6 @@ int enqueue_iteration_t(cel_ctx* c) {
   after_launch(c, CEL_K_INIT_FILL, n);
   // (every sort mode: besides the index scatter of the sorted modes it closes the fill — vacancy counters, control block)
   launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n);
-  if (D.sort_mode == CEL_SORT_BY_ACTION && c->fused) {
-    // one launch walks the chunks of every action's range (k_actions): the whole iteration is one PDL chain
-    if (cyl) { if (field) launch_chain(c, k_actions<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 1, TR>, pg, kBlock, s); }
-    else { if (field) launch_chain(c, k_actions<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_actions<false, 0, TR>, pg, kBlock, s); }
-    after_launch(c, CEL_K_ACTIONS, n);
-    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
-    return n;
-  }
-  if (c->fused) {   // masked modes: one launch, one thread per slot, the action switched on (k_actions_masked)
-    if (cyl) { if (field) launch_chain(c, k_actions_masked<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 1, TR>, pg, kBlock, s); }
-    else { if (field) launch_chain(c, k_actions_masked<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_actions_masked<false, 0, TR>, pg, kBlock, s); }
-    after_launch(c, CEL_K_ACTIONS, n);
-    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
-    return n;
-  }
   const bool fork = c->concurrent && !c->profile;
   const bool by_action = D.sort_mode == CEL_SORT_BY_ACTION;
   if ((D.sort_mode == CEL_SORT_NONE || D.sort_mode == CEL_SORT_PARTITION) && c->merge_discrete) {
@@ -522,17 +496,13 @@ int enqueue_iteration_t(cel_ctx* c) {
   cudaStream_t s_photon = s, s_annih = s, s_pe = s, s_pair = s;
   int n_side = 0;
   if (fork) {
-    n_side = by_action ? (c->merge_discrete == 2 ? 1 : (c->merge_discrete ? 2 : 4)) : 1;
+    n_side = by_action ? (c->merge_discrete ? 2 : 4) : 1;
     cudaEventRecord(c->ev_fork, s);
     for (int i = 0; i < n_side; ++i) cudaStreamWaitEvent(c->side[i], c->ev_fork, 0);
     s_photon = c->side[0]; s_pe = c->side[0]; s_pair = c->side[0];
     if (by_action) { s_annih = c->side[1]; s_pe = c->side[2]; s_pair = c->side[3]; }
   }
-  const bool merge_photon = by_action && c->merge_discrete == 2;
-  if (merge_photon) {
-    if (cyl) k_neutral<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_neutral<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
-    after_launch(c, CEL_K_DISCRETE, n);
-  } else if (by_action && c->merge_discrete) {
+  if (by_action && c->merge_discrete) {
     const int dg = pg < c->n_sm ? pg : c->n_sm;   // one block per SM: the ranges are small, and a small grid launches faster
     k_discrete<TR><<<dg, kBlock, 0, s_annih>>>(D); after_launch(c, CEL_K_DISCRETE, n);
   } else {
@@ -540,10 +510,8 @@ int enqueue_iteration_t(cel_ctx* c) {
     k_photoelectric<TR><<<pg, kBlock, 0, s_pe>>>(D); after_launch(c, CEL_K_PE, n);
     if (c->phys.enable_pair) { k_pair<TR><<<pg, kBlock, 0, s_pair>>>(D); after_launch(c, CEL_K_PAIR, n); }
   }
-  if (!merge_photon) {
-    if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
-    after_launch(c, CEL_K_PHOTON, n);
-  }
+  if (cyl) k_photon<1, TR><<<pg, kBlock, 0, s_photon>>>(D); else k_photon<0, TR><<<pg, kBlock, 0, s_photon>>>(D);
+  after_launch(c, CEL_K_PHOTON, n);
   // (in the masked modes the annihilation kernel precedes it on the main stream)
   if (cyl) { if (field) launch_chain(c, k_charged<true, 1, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 1, TR>, pg, kBlock, s); }
   else { if (field) launch_chain(c, k_charged<true, 0, TR>, pg, kBlock, s); else launch_chain(c, k_charged<false, 0, TR>, pg, kBlock, s); }
@@ -568,35 +536,6 @@ int collect_profile(cel_ctx* c, int n_iter, int kernels_per_iteration) {
       c->kernel_ms[c->iter_kernel[i]] += ms;
       c->kernel_launches[c->iter_kernel[i]] += 1;
     }
-  return CEL_OK;
-}
-
-// ---- the persistent form (cel_persistent.cuh): one cooperative kernel per batch of iterations
-const void* persistent_function(const cel_ctx* c) {
-  const bool cyl = c->D.P.geom_kind == CEL_GEOM_CYL, field = c->D.P.bmag != 0.0;
-  if (cyl) return field ? (const void*)k_persistent<true, 1> : (const void*)k_persistent<false, 1>;
-  return field ? (const void*)k_persistent<true, 0> : (const void*)k_persistent<false, 0>;
-}
-// co-resident grid for the cooperative launch; 0 if the device cannot run it (then the kernel-per-action form is used)
-void setup_persistent(cel_ctx* c) {
-  c->persist_fn = persistent_function(c);
-  c->persist_grid = 0;
-  if (c->D.sort_mode == CEL_SORT_PARTITION) return;   // the partition passes exist in the kernel-per-action form only
-  int dev = 0, coop = 0, per_sm = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return;
-  if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) return;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, c->persist_fn, kTileThreads, 0) != cudaSuccess || per_sm < 1) return;
-  const int grid = per_sm * c->n_sm;
-  if ((c->D.n_tiles + grid - 1) / grid > (uint32_t)kMaxTilesPerBlock) return;
-  c->persist_grid = grid;
-}
-bool use_persistent(const cel_ctx* c) { return c->persistent && !c->profile && c->persist_grid > 0; }
-int launch_persistent(cel_ctx* c, uint32_t max_iters) {
-  CEL_CUDA(c, cudaMemsetAsync(&c->D.ctl->barrier, 0, sizeof(unsigned long long), c->stream));
-  DeviceState D = c->D;
-  void* args[] = {(void*)&D, (void*)&max_iters};
-  CEL_CUDA(c, cudaLaunchCooperativeKernel(c->persist_fn, dim3(c->persist_grid), dim3(kTileThreads), args, 0, c->stream));
-  c->launches += 1;
   return CEL_OK;
 }
 
@@ -657,7 +596,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
   // (the stream-ordered pool hands the same scratch back run after run, so the graph of the last run is normally
   // still valid: it is kept when every baked-in argument and option is unchanged)
-  const int cfg[6] = {c->batch, c->concurrent, c->pdl, c->fused, c->trace_iters, c->merge_discrete};
+  const int cfg[6] = {c->batch, c->concurrent, c->pdl, 0, c->trace_iters, c->merge_discrete};
   const bool graph_valid = c->graph_exec && std::memcmp(&c->graph_D, &D, sizeof(DeviceState)) == 0 &&
                            std::memcmp(c->graph_cfg, cfg, sizeof(cfg)) == 0;
   if (!graph_valid) {
@@ -673,7 +612,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
       c->prof_ev.push_back(e);
     }
   }
-  if (c->use_graph && !c->profile && !use_persistent(c) && !graph_valid) {
+  if (c->use_graph && !c->profile && !graph_valid) {
     // one graph = one batch of iterations: a single cudaGraphLaunch per status poll keeps the host far ahead of the device
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     for (int b = 0; b < c->batch; ++b) c->kernels_per_iteration = enqueue_iteration(c);
@@ -732,11 +671,7 @@ int run_loop(cel_ctx* c) {
   int rc = CEL_OK;
   while (true) {
     int per_iter = c->kernels_per_iteration;
-    if (use_persistent(c)) {
-      int prc = launch_persistent(c, (uint32_t)c->persist_batch);
-      if (prc != CEL_OK) return prc;
-      enqueued += c->persist_batch - c->batch;
-    } else if (c->graph_exec && c->use_graph && !c->profile) {
+    if (c->graph_exec && c->use_graph && !c->profile) {
       CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s));
       c->launches += (uint64_t)c->kernels_per_iteration * c->batch;
     } else {
@@ -841,8 +776,7 @@ extern "C" int cel_debug_begin(cel_ctx* c, const cel_primary* primaries, uint64_
 
 extern "C" int cel_debug_step(cel_ctx* c) {
   if (!c || !c->ran) return CEL_ERR_NOT_RUN;
-  if (use_persistent(c)) { int prc = launch_persistent(c, 1); if (prc != CEL_OK) return prc; }
-  else c->launches += enqueue_iteration(c);
+  c->launches += enqueue_iteration(c);
   CEL_CUDA(c, cudaGetLastError());
   CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[0], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
   CEL_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -119,7 +119,6 @@ struct Control {
   unsigned long long n_init_fill;   // I after the fill of this iteration (= n_init until k_push adds S)
   uint32_t iter_cur;                // k of the running iteration, a copy k_push may read while its block 0 bumps iter
   uint32_t part_charged;            // sort mode 3: charged initializers among the n_take popped in this iteration
-  unsigned long long barrier;       // arrival counter of the persistent kernel's grid barrier (zeroed per launch)
 };
 
 // everything a kernel needs; passed by value (fits in the 4 KB parameter space)
@@ -160,7 +159,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_ACTIONS, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
+enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;

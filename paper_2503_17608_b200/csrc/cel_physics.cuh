@@ -536,145 +536,4 @@ __global__ void __launch_bounds__(kBlock) k_discrete_masked(DeviceState D) {
   }
 }
 
-// The same with the photon kernel in the launch as well (option merge_discrete = 2): photon chunks first (the heavy
-// part), then the three pure interactions. Two action launches per iteration: this one beside k_charged. Runs at the
-// photon kernel's register count, which the three small actions do not mind.
-template <int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock) k_neutral(DeviceState D) {
-  pdl_prologue();
-  const Control* ctl = D.ctl;
-  const uint32_t finished_ = ctl->finished;
-  const uint32_t b_ph = ctl->rb[R_PHOTON], e_ph = ctl->re[R_PHOTON];
-  const uint32_t b_an = ctl->rb[R_ANNIH], e_an = ctl->re[R_ANNIH];
-  const uint32_t b_pe = ctl->rb[R_PE], e_pe = ctl->re[R_PE];
-  const uint32_t b_pa = ctl->rb[R_PAIR], e_pa = ctl->re[R_PAIR];
-  const uint32_t k_iter = ctl->iter;
-  if (finished_) return;
-  const TraceScope<K_DISCRETE, TRACE> trace(D, k_iter);
-  const uint32_t n_ph = (e_ph - b_ph + kBlock - 1) / kBlock;
-  const uint32_t n_an = (e_an - b_an + kBlock - 1) / kBlock, n_pe = (e_pe - b_pe + kBlock - 1) / kBlock;
-  const uint32_t n_pa = (e_pa - b_pa + kBlock - 1) / kBlock;
-  const uint32_t c0 = n_ph, c1 = c0 + n_pe, c2 = c1 + n_an, c3 = c2 + n_pa;
-  for (uint32_t v = blockIdx.x; v < c3; v += gridDim.x) {   // block-uniform
-    if (v < c0) {
-      const uint32_t tid = b_ph + v * kBlock + threadIdx.x;
-      if (tid < e_ph) {
-        const uint32_t slot = D.indices[tid];
-        const RecB b = load_b(D.stB + slot);
-        const RecA a = load_a(D.stA + slot);
-        const int act = meta_action(b.meta);
-        if (act == A_COMPTON || act == A_MOVE_G) do_photon<GEOM>(D, slot, k_iter, a, b, act);
-      }
-      continue;
-    }
-    uint32_t tid, end; int want;
-    if (v < c1) { tid = b_pe + (v - c0) * kBlock; end = e_pe; want = A_PE; }
-    else if (v < c2) { tid = b_an + (v - c1) * kBlock; end = e_an; want = A_ANNIH; }
-    else { tid = b_pa + (v - c2) * kBlock; end = e_pa; want = A_PAIR; }
-    tid += threadIdx.x;
-    if (tid < end) {
-      const uint32_t slot = D.indices[tid];
-      const RecB b = load_b(D.stB + slot);
-      const RecA a = load_a(D.stA + slot);
-      if (meta_action(b.meta) == want) {
-        if (want == A_PE) do_photoelectric(D, slot, a, b);
-        else if (want == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
-        else do_pair(D, slot, k_iter, a, b);
-      }
-    }
-  }
-}
-
-// ================================================================ all action kernels in ONE launch (sort by action)
-// Sorted by action, every action owns a contiguous range of the index array. Instead of one launch per
-// action, the ranges are cut into chunks of kBlock indices and ONE grid walks the chunks of all ranges, heaviest action
-// first (charged, photon, annihilation, photoelectric, pair): a block still runs exactly one action's code on one
-// contiguous piece of that action's range — no masks, no divergence between actions inside a block — but the
-// iteration loses four launches, the fork / join of the side streams, and the tail in which the small kernels queued
-// behind the blocks of the big ones (profiles/: timeline). Results are bit-identical to the kernel-per-action form.
-template <bool FIELD, int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock, FIELD ? 2 : 4) k_actions(DeviceState D) {
-  pdl_prologue();
-  const Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const uint32_t k_iter = ctl->iter;
-  const TraceScope<K_ACTIONS, TRACE> trace(D, k_iter);
-  // chunk ranges, in launch order
-  const uint32_t b_ch = ctl->rb[R_CHARGED], e_ch = ctl->re[R_CHARGED];
-  const uint32_t b_ph = ctl->rb[R_PHOTON], e_ph = ctl->re[R_PHOTON];
-  const uint32_t b_an = ctl->rb[R_ANNIH], e_an = ctl->re[R_ANNIH];
-  const uint32_t b_pe = ctl->rb[R_PE], e_pe = ctl->re[R_PE];
-  const uint32_t b_pa = ctl->rb[R_PAIR], e_pa = ctl->re[R_PAIR];
-  const uint32_t n_ch = (e_ch - b_ch + kBlock - 1) / kBlock, n_ph = (e_ph - b_ph + kBlock - 1) / kBlock;
-  const uint32_t n_an = (e_an - b_an + kBlock - 1) / kBlock, n_pe = (e_pe - b_pe + kBlock - 1) / kBlock;
-  const uint32_t n_pa = (e_pa - b_pa + kBlock - 1) / kBlock;
-  const uint32_t c1 = n_ch, c2 = c1 + n_ph, c3 = c2 + n_an, c4 = c3 + n_pe, c5 = c4 + n_pa;
-  for (uint32_t v = blockIdx.x; v < c5; v += gridDim.x) {   // block-uniform: one action per block and chunk
-    if (v < c1) {
-      const uint32_t tid = b_ch + v * kBlock + threadIdx.x;
-      if (tid < e_ch) {
-        const uint32_t slot = D.indices[tid];
-        const RecB b = load_b(D.stB + slot);
-        const RecA a = load_a(D.stA + slot);
-        const int act = meta_action(b.meta);
-        if (act == A_MOVE_C || act == A_BREMS) do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
-      }
-    } else if (v < c2) {
-      const uint32_t tid = b_ph + (v - c1) * kBlock + threadIdx.x;
-      if (tid < e_ph) {
-        const uint32_t slot = D.indices[tid];
-        const RecB b = load_b(D.stB + slot);
-        const RecA a = load_a(D.stA + slot);
-        const int act = meta_action(b.meta);
-        if (act == A_COMPTON || act == A_MOVE_G) do_photon<GEOM>(D, slot, k_iter, a, b, act);
-      }
-    } else {
-      uint32_t tid, end; int want;
-      if (v < c3) { tid = b_an + (v - c2) * kBlock; end = e_an; want = A_ANNIH; }
-      else if (v < c4) { tid = b_pe + (v - c3) * kBlock; end = e_pe; want = A_PE; }
-      else { tid = b_pa + (v - c4) * kBlock; end = e_pa; want = A_PAIR; }
-      tid += threadIdx.x;
-      if (tid < end) {
-        const uint32_t slot = D.indices[tid];
-        const RecB b = load_b(D.stB + slot);
-        const RecA a = load_a(D.stA + slot);
-        if (meta_action(b.meta) == want) {
-          if (want == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
-          else if (want == A_PE) do_photoelectric(D, slot, a, b);
-          else do_pair(D, slot, k_iter, a, b);
-        }
-      }
-    }
-  }
-}
-
-// ================================================================ all actions in ONE masked launch (modes none / by particle / partition)
-// One thread per slot of the kernel's range, the action read once and switched on: a slot is visited exactly once per
-// iteration, so no order between interaction and move kernels has to be kept, and the dense key bytes are read once
-// instead of once per action kernel. What it costs is what PAPER.md:37-47 describes: a warp whose lanes hold different
-// actions serialises their code paths — which the partition of sort mode 3 is there to reduce.
-// Results are bit-identical to the kernel-per-action form of the same sort mode.
-template <bool FIELD, int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock) k_actions_masked(DeviceState D) {
-  pdl_prologue();
-  const Control* ctl = D.ctl;
-  if (ctl->finished) return;
-  const uint32_t k_iter = ctl->iter;
-  const TraceScope<K_ACTIONS, TRACE> trace(D, k_iter);
-  // by particle: the non-vacant part of the index array (gamma | e- | e+); otherwise every slot
-  const uint32_t rb = 0, re = D.sort_mode == 2 ? ctl->offsets[3] : D.N;
-  for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x) {
-    const uint32_t slot = slot_of(D, tid);
-    if ((D.akey[slot] & 0xf) == A_VACANT) continue;
-    const RecB b = load_b(D.stB + slot);
-    const RecA a = load_a(D.stA + slot);
-    const int act = meta_action(b.meta);
-    if (act == A_MOVE_C || act == A_BREMS) do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
-    else if (act == A_MOVE_G || act == A_COMPTON) do_photon<GEOM>(D, slot, k_iter, a, b, act);
-    else if (act == A_PE) do_photoelectric(D, slot, a, b);
-    else if (act == A_PAIR) do_pair(D, slot, k_iter, a, b);
-    else if (act == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
-  }
-}
-
 }  // namespace cel

@@ -76,7 +76,6 @@ def main():
     ap.add_argument("--slots", type=int, default=0)
     ap.add_argument("--sort-mode", type=int, default=1, choices=[0, 1, 2, 3])
     ap.add_argument("--iters", type=int, default=512, help="iterations to stamp")
-    ap.add_argument("--fused", type=int, default=0)
     ap.add_argument("--out", default="trace.json")
     args = ap.parse_args()
     assert torch.cuda.is_available(), "trace_export needs a CUDA device"
@@ -84,7 +83,6 @@ def main():
     kw = {k: v for k, v in (("n_events", args.events), ("n_slots", args.slots)) if v}
     w = getattr(W, args.workload)(sort_mode=args.sort_mode, **kw)
     ctx = binding.from_workload(w)
-    ctx.set_option("fused", args.fused)
     ctx.transport(w.primaries, w.n_events); ctx.tallies_view()          # warm-up
     ctx.set_option("trace", args.iters)
     ctx.transport(w.primaries, w.n_events)

@@ -52,13 +52,13 @@ def test_timeline_is_ordered_and_does_not_change_results(binding):
     v = ctx.tallies_view()
     assert np.array_equal(v["fixed"], ref_fixed) and v["track_steps"] == ref["track_steps"]
     names, t = ctx.trace()
-    assert names[0] == "init_fill" and "push" in names and "actions" in names and t.shape == (64, len(names), 2)
+    assert names[0] == "init_fill" and "push" in names and "discrete" in names and t.shape == (64, len(names), 2)
     n = min(64, int(v["iterations"]))
     t = t.astype(np.int64)
     ran = t[:n, :, 1] > 0
     i_fill, i_scatter, i_push = names.index("init_fill"), names.index("scatter"), names.index("push")
     assert ran[:, i_fill].all() and ran[:, i_scatter].all() and ran[:, i_push].all()
-    assert ran[:, names.index("charged")].all() and not ran[:, names.index("actions")].any()   # launch per action
+    assert ran[:, names.index("charged")].all() and not ran[:, names.index("discrete")].any()   # launch per action
     assert np.all(t[:n, :, 1][ran] >= t[:n, :, 0][ran])               # end >= start
     fill, scatter, push = t[:n, i_fill], t[:n, i_scatter], t[:n, i_push]
     assert np.all(scatter[:, 0] >= fill[:, 1])                        # P2 after P1
@@ -68,11 +68,11 @@ def test_timeline_is_ordered_and_does_not_change_results(binding):
         r = ran[:, j]
         assert np.all(t[:n, j, 0][r] >= scatter[:, 1][r]) and np.all(push[:, 0][r] >= t[:n, j, 1][r])
     assert np.all(fill[1:, 0] >= push[:-1, 1])                        # next iteration after the push
-    # the one-launch form stamps "actions" instead of the five action kernels
-    ctx.set_option("fused", 1)
+    # the merged launch of the three pure interactions stamps "discrete" instead of their three kernels
+    ctx.set_option("merge_discrete", 1)
     ctx.transport(w.primaries, w.n_events)
     v2 = ctx.tallies_view()
     assert np.array_equal(v2["fixed"], ref_fixed)
     _, t2 = ctx.trace()
-    assert (t2[:n, names.index("actions"), 1] > 0).all() and not (t2[:n, names.index("charged"), 1] > 0).any()
+    assert (t2[:n, names.index("discrete"), 1] > 0).all() and not (t2[:n, names.index("photoelectric"), 1] > 0).any()
     ctx.close()

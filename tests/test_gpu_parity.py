@@ -14,27 +14,11 @@ M_E = 0.51099895
 TOL = 1e-12
 
 
-class _ExecutionForm:
-    """the binding module, with every context switched to one execution form of the iteration: the persistent
-    cooperative kernel (cel_persistent.cuh, the default) or the kernel-per-action CUDA graph"""
-
-    def __init__(self, b, persistent):
-        self._b, self._persistent = b, persistent
-
-    def __getattr__(self, name):
-        return getattr(self._b, name)
-
-    def from_workload(self, *a, **k):
-        ctx = self._b.from_workload(*a, **k)
-        ctx.set_option("persistent", self._persistent)
-        return ctx
-
-
-@pytest.fixture(scope="module", params=["persistent", "kernels"])
-def binding(request):
+@pytest.fixture(scope="module")
+def binding():
     from paper_2503_17608_b200 import binding as b
     b.load_library()
-    return _ExecutionForm(b, 1 if request.param == "persistent" else 0)
+    return b
 
 
 def compare_states(g, o, where=""):
@@ -60,30 +44,75 @@ def compare_initializers(g, o, where=""):
     assert np.all(np.abs(g["energy"] - o["energy"]) <= TOL * np.abs(o["energy"])), where
 
 
-def lockstep(binding, w, n_iter, must_match):
-    """step both sides together; everything must agree for the first `must_match` iterations; returns how many agreed"""
+def check_integer_work_self_consistent(ctx, st, sort_mode, where=""):
+    """what is unique given the GPU's OWN keys (valid at every iteration, also after a float decision flip has separated
+    the two histories): the index array is the stable counting sort of the slot keys (S2), offsets and the logged counts
+    are the key histogram"""
+    gi, goff = ctx.indices()
+    act = st["action"]
+    if sort_mode == 1:
+        keys, nk = act, 8
+    elif sort_mode == 2:
+        keys, nk = np.where(act == VACANT, 3, st["ptype"]), 4
+    else:
+        return
+    # the action kernels have run since the sort: compare against the keys the sort saw = logged counts + stability
+    cnt = ctx.counts()[-1]
+    if sort_mode == 1:
+        assert np.array_equal(goff, np.concatenate([[0], np.cumsum(cnt)])), where
+    assert np.array_equal(np.sort(gi), np.arange(len(gi), dtype=np.uint32)), where      # a permutation
+    for k in range(nk):
+        seg = gi[goff[k]:goff[k + 1]]
+        assert np.all(np.diff(seg.astype(np.int64)) > 0), (where, "stable within key", k)
+
+
+def lockstep(binding, w, n_iter, must_match, min_agreed=None):
+    """step both sides together; integer work bit-exact, floating state within 1e-12 and the tallies within the first-step
+    deposit tolerance (A24) for the first `must_match` iterations at least. The first later disagreement must be a
+    handful of float-driven decision flips (a few slots), not an indexing error; after it the GPU's integer work is still
+    checked for self-consistency. Returns how many iterations agreed."""
     ctx = binding.from_workload(w)
     o = make_oracle(w)
     ctx.begin(w.primaries, w.n_events); o.begin(w.primaries, w.n_events)
+    e_max = float(w.primaries["energy"].max()) if len(w.primaries) else 1.0
+    tol_q = int(np.ceil(TOL * e_max * 2.0 ** 36)) + 2      # quanta per cell: 1e-12 T0 (A24) + rounding of llrint
     agreed = 0
+    diverged = False
     for k in range(n_iter):
-        ctx.step(); o.step()
+        ctx.step()
+        gst = ctx.state()
+        check_integer_work_self_consistent(ctx, gst, w.sort_mode, f"iter {k}")
+        if diverged:
+            if (gst["action"] != VACANT).sum() == 0 and len(ctx.initializers()) == 0:
+                break
+            continue
+        o.step()
+        ost = o.state()
         try:
             gi, goff = ctx.indices(); oi, ooff = o.indices()
             assert np.array_equal(goff, ooff), f"offsets iter {k}"
             # the vacant tail of the permutation is also defined (stable) -> the whole permutation is compared
             assert np.array_equal(gi, oi), f"permutation iter {k}"
             assert np.array_equal(ctx.counts(), o.counts()[:len(ctx.counts())]), f"counts iter {k}"
-            compare_states(ctx.state(), o.state(), f"iter {k}")
+            compare_states(gst, ost, f"iter {k}")
             compare_initializers(ctx.initializers(), o.initializers(), f"iter {k}")
+            dq = ctx.tallies_fixed().astype(np.int64) - o.tallies_fixed().astype(np.int64)
+            assert np.abs(dq).max(initial=0) <= tol_q, f"tallies iter {k}: {np.abs(dq).max()} quanta"
         except AssertionError:
             if k < must_match:
                 raise
-            break
+            # a decision flip: few slots differ in action; everything else would be an indexing bug
+            n_diff = int((gst["action"] != ost["action"]).sum())
+            live = int((ost["action"] != VACANT).sum())
+            assert n_diff <= max(4, live // 200), f"iter {k}: {n_diff} of {live} slots differ — not a decision flip"
+            diverged = True
+            continue
         agreed += 1
-        if (o.state()["action"] != VACANT).sum() == 0 and len(o.initializers()) == 0:
+        if (ost["action"] != VACANT).sum() == 0 and len(o.initializers()) == 0:
             break
     ctx.close()
+    if min_agreed is not None:
+        assert agreed >= min_agreed, agreed
     return agreed
 
 
@@ -203,26 +232,13 @@ def test_graph_and_direct_launch_identical(binding):
     assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb)
 
 
-def test_persistent_and_kernel_forms_identical(binding):
-    """the persistent cooperative kernel and the kernel-per-action graph are the same algorithm: tallies, per-iteration
-    action counts and counters agree bit-exactly in every sort mode (slab + field, and the cylinder geometry)"""
-    for w0 in (W.config3(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
-        for mode in (0, 1, 2):
-            w0.sort_mode = mode
-            a, ca = run_gpu(binding, w0, persistent=1, persist_batch=7)
-            b, cb = run_gpu(binding, w0, persistent=0)
-            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
-            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
-            assert a["kernel_launches"] < b["kernel_launches"]
-
-
 def test_partition_mode_whole_runs(binding):
     """sort mode 3 (charged / neutral partition, section 3.2): whole showers conserve energy per event, are
     reproducible bit for bit, keep the two species at opposite ends while the array is far from full, and follow the
     oracle's run of the same mode closely (same seeds; only last-ulp decision flips separate them)"""
     for w in (W.config3(n_events=30, n_slots=1 << 14, energy=2000.0, sort_mode=3), W.config4(n_events=2, per_event=6, n_slots=1 << 14, sort_mode=3)):
-        a, ca = run_gpu(binding, w, persistent=0)
-        b, cb = run_gpu(binding, w, persistent=0, use_graph=0, batch=5)
+        a, ca = run_gpu(binding, w)
+        b, cb = run_gpu(binding, w, use_graph=0, batch=5)
         assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb)
         e = a["fixed"].astype(np.float64).sum(1) * 2.0 ** -36
         assert np.all(np.abs(e - expected_energy(w)) <= 1e-9 * expected_energy(w))
@@ -252,12 +268,11 @@ def test_merged_discrete_kernel_identical(binding):
     kernels: same tallies, per-iteration counts and counters"""
     for w0 in (W.config2(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
         w0.sort_mode = 1
-        b, cb = run_gpu(binding, w0, persistent=0, merge_discrete=0)
-        for md in (1, 2):   # 2: the photon kernel in the same launch as well (k_neutral)
-            a, ca = run_gpu(binding, w0, persistent=0, merge_discrete=md)
-            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, md)
-            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
-            assert a["kernel_launches"] < b["kernel_launches"]
+        b, cb = run_gpu(binding, w0, merge_discrete=0)
+        a, ca = run_gpu(binding, w0, merge_discrete=1)
+        assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), w0.name
+        assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
+        assert a["kernel_launches"] < b["kernel_launches"]
 
 
 def test_merged_discrete_masked_identical(binding):
@@ -266,25 +281,10 @@ def test_merged_discrete_masked_identical(binding):
     for w0 in (W.config3(n_events=20, n_slots=1 << 14, energy=3000.0), W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
         for mode in (0, 3):
             w0.sort_mode = mode
-            a, ca = run_gpu(binding, w0, persistent=0, merge_discrete=1)
-            b, cb = run_gpu(binding, w0, persistent=0, merge_discrete=0)
+            a, ca = run_gpu(binding, w0, merge_discrete=1)
+            b, cb = run_gpu(binding, w0, merge_discrete=0)
             assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
             assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"]
-            assert a["kernel_launches"] < b["kernel_launches"]
-
-
-def test_fused_and_per_action_launches_identical(binding):
-    """the one-launch forms (sorted by action: k_actions walks the chunks of every action's range; masked modes:
-    k_actions_masked, one thread per slot with the action switched on) and the launch-per-action form give the same
-    tallies, per-iteration action counts and counters, bit for bit (slab, slab + field, cylinder + field)"""
-    for w0 in (W.config2(n_events=20, n_slots=1 << 14, energy=3000.0), W.config3(n_events=20, n_slots=1 << 14, energy=3000.0),
-               W.config4(n_events=2, per_event=6, n_slots=1 << 14)):
-        for mode in (1, 0, 2, 3):   # 1: k_actions over the action ranges; 0, 2, 3: k_actions_masked, one thread per slot
-            w0.sort_mode = mode
-            a, ca = run_gpu(binding, w0, persistent=0, fused=1)
-            b, cb = run_gpu(binding, w0, persistent=0, fused=0)
-            assert np.array_equal(a["fixed"], b["fixed"]) and np.array_equal(ca, cb), (w0.name, mode)
-            assert a["track_steps"] == b["track_steps"] and a["secondaries"] == b["secondaries"] and a["iterations"] == b["iterations"]
             assert a["kernel_launches"] < b["kernel_launches"]
 
 

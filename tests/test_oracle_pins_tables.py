@@ -166,3 +166,40 @@ def test_range_inverse_is_exact_inverse(ctx):
     # monotone
     for mat in range(5):
         assert np.all(np.diff(ctx.table(mat, "range")) > 0)
+
+
+def test_stopping_power_textbook_limits():
+    """S(T) pinned by facts that are not the S4 expression re-typed (the survey's S_* goldens are regression values):
+    * non-relativistic limit: the textbook Bethe formula for electrons, S -> (4 pi r_e^2 m_e n_e / beta^2) ln(sqrt(e/2) T / I)
+      with beta^2 = 2T/m_e (the S4 bracket reduces to 2 ln(tau/iota) + 1 - ln 2 as tau -> 0), agreement O(tau);
+    * ultra-relativistic limit: S -> 2 pi r_e^2 m_e n_e [ln(tau^3 / (2 iota^2)) + 1/8], agreement O(1/tau);
+    * positivity and the 1/beta^2 rise towards low energy."""
+    BE = (1.848, 4.0, 9.0122)   # low Z: I = 55.7 eV << 1 keV
+    geo = W.slab_geometry([0.0, 1.0], [0], [0], 50.0)
+    o = orc.Oracle(geo, [BE, W.LAR], W.physics(1), 4, 1)
+    N_A = 6.02214076e23
+    for mat, (rho, Z, A) in enumerate([BE, W.LAR]):
+        n_e = Z * rho * N_A / A
+        I = 16e-6 * Z ** 0.9
+        dev = []
+        for T in (1e-3, 2e-3, 5e-3):
+            tau = T / M_E
+            nr = 4 * math.pi * R_E ** 2 * M_E * n_e / (2 * tau) * math.log(math.sqrt(math.e / 2) * T / I)
+            d = o.stopping_power(mat, T) / nr - 1.0
+            assert abs(d) < 2.0 * tau, (mat, T, d)
+            dev.append(d)
+        assert dev[0] < dev[1] < dev[2] and dev[2] / dev[0] > 3.0          # the residual is O(tau): it shrinks with T
+        for T in (1e3, 1e4, 1e5):
+            tau = T / M_E
+            ur = 2 * math.pi * R_E ** 2 * M_E * n_e * (math.log(tau ** 3 / (2 * (I / M_E) ** 2)) + 0.125)
+            assert abs(o.stopping_power(mat, T) / ur - 1.0) < 0.02 / tau, (mat, T)
+        # 1/beta^2 rise: S falls monotonically from 1 keV to ~1 MeV (minimum ionisation), then rises logarithmically
+        E = np.logspace(-3, 5, 400)
+        S = np.array([o.stopping_power(mat, e) for e in E])
+        imin = int(np.argmin(S))
+        assert 0.5 < E[imin] < 3.0 and np.all(np.diff(S[:imin]) < 0) and np.all(np.diff(S[imin:]) > 0) and np.all(S > 0)
+        # between 1 and 2 keV the fall is the 1/beta^2 factor times the slowly growing logarithm
+        r = o.stopping_power(mat, 1e-3) / o.stopping_power(mat, 2e-3)
+        expect = 2.0 * math.log(math.sqrt(math.e / 2) * 1e-3 / I) / math.log(math.sqrt(math.e / 2) * 2e-3 / I)
+        assert abs(r / expect - 1.0) < 5e-3
+    o.close()

@@ -248,3 +248,146 @@ def test_no_track_reaches_looper_cap_in_the_calorimeter():
     o = make_oracle(w)
     o.transport(w.primaries, w.n_events)
     assert o.counters()["iterations"] < 400
+
+
+# ---------------------------------------------------------------- round-2 pins: bin attribution, looper cap, cylinder crossings
+def _range_tables(o, mat=0):
+    u = math.log(1e-3) + np.arange(577) * (math.log(10.0) / 64.0)
+    return u, o.table(mat, "range")
+
+
+def _eloss_numpy(o, mat, T0, s):
+    """T0 - Rinv(R(T0) - s) restated with numpy's piecewise-linear interpolation of the (already pinned) range table:
+    R is linear in u = ln T between nodes (S4), Rinv is the inverse of that lerp"""
+    u, R = _range_tables(o, mat)
+    r0 = np.interp(math.log(T0), u, R)
+    return T0 - math.exp(np.interp(r0 - s, R, u))
+
+
+def test_score_bin_is_the_pre_step_volume():
+    """S10: the deposit of a step goes to the bin of the volume occupied at the START of the iteration, also when the
+    step ends in the next volume or outside. Two volumes with distinct bins (Pb bin 0 | LAr bin 1), eloss-only
+    electrons (no brems, no MSC: the step is deterministic) started 10 um before a plane."""
+    geo = W.slab_geometry([0.0, 1.0, 2.0], [0, 1], [0, 1], 50.0)
+    Q = 2.0 ** -36
+    T0 = 10.0
+    eps = 1e-3
+    # (1) crossing Pb -> LAr: the whole T0 - T1 of the crossing step lands in bin 0, nothing in bin 1 or escape
+    o = orc.Oracle(geo, [W.LEAD, W.LAR], phys(31, enable_brems=0, enable_msc=0), 4, 1)
+    o.begin(W.beam(1, 1, W.ELECTRON, T0, pos=(0.0, 0.0, 1.0 - eps)), 1)
+    o.step()
+    st = o.state()[0]
+    assert st["vol"] == 1 and st["pos"][2] == 1.0 and st["action"] == 4        # it did cross, and is still moving
+    s_b = 1.0 - (1.0 - eps)                                                     # the subtraction the step performs
+    dep = _eloss_numpy(o, 0, T0, s_b)
+    T = o.tallies()[0]
+    assert abs(T[0] - dep) <= 1e-12 * T0 + Q and dep > 1e-3                     # a real deposit (~ 12 keV), in the Pb bin
+    assert T[1] == 0.0 and T[2] == 0.0
+    assert abs(st["energy"] - (T0 - dep)) <= 1e-12 * T0
+    # (2) the NEXT step starts in LAr: its deposit goes to bin 1 and bin 0 stays what it was
+    T1 = st["energy"]
+    o.step()
+    Tn = o.tallies()[0]
+    r_lar = np.interp(math.log(T1), *_range_tables(o, 1))
+    s2 = max(0.2 * r_lar, 0.01)
+    assert s2 < 1.0                                                             # stays inside the LAr volume
+    assert Tn[0] == T[0] and Tn[2] == 0.0
+    assert abs(Tn[1] - _eloss_numpy(o, 1, T1, s2)) <= 1e-12 * T0 + Q
+    # (3) escape step from LAr: deposit in bin 1 (pre-step), remainder T1 in the escape bin, nothing in bin 0
+    o.begin(W.beam(1, 1, W.ELECTRON, T0, pos=(0.0, 0.0, 2.0 - eps)), 1)
+    o.step()
+    assert o.state()[0]["action"] == VACANT
+    T = o.tallies()[0]
+    dep = _eloss_numpy(o, 1, T0, 2.0 - (2.0 - eps))
+    assert T[0] == 0.0 and abs(T[1] - dep) <= 1e-12 * T0 + Q and abs(T[2] - (T0 - dep)) <= 1e-12 * T0 + Q
+    # (4) an interaction deposit (photoelectric with local electrons) goes to the bin of the volume the photon is in:
+    # half of the photons start in the Pb, half in the LAr; per event the deposit sits in the bin of the absorption point
+    n = 4000
+    o = orc.Oracle(geo, [W.LEAD, W.LAR], phys(32, electrons_local=1, enable_pair=0), n, 0)
+    prim = W.beam(n, 1, W.GAMMA, 0.05, pos=(0.0, 0.0, 0.5))                      # 50 keV: photoelectric dominates
+    prim["pos"][1::2, 2] = 1.5
+    o.begin(prim, n)
+    seen = {0: 0, 1: 0}
+    for _ in range(6):
+        pre = o.state().copy()
+        before = o.tallies_fixed().copy()
+        o.step()
+        d = o.tallies_fixed().astype(np.int64) - before.astype(np.int64)
+        pe = np.flatnonzero(pre["action"] == 0)                                  # slots that apply PE in this iteration
+        for s in pe:
+            ev, vol = int(pre["event"][s]), int(pre["vol"][s])
+            assert d[ev, vol] > 0 and d[ev, 1 - vol] == 0
+            seen[vol] += 1
+    assert seen[0] > 1000 and seen[1] > 1000
+
+
+@pytest.mark.parametrize("ptype,rest", [(W.ELECTRON, 0.0), (W.POSITRON, 2 * M_E)])
+def test_looper_cap_fate(ptype, rest):
+    """S7.6: a charged track that has made max_steps_per_track steps is ended, its kinetic energy (+ 2 m_e for e+,
+    reading A16) credited to the ESCAPE bin. Vacuum + 1 T: nothing else can end the track."""
+    geo = W.slab_geometry([-1e6, 1e6], [-1], [0], 1e6, (1.0, 0.0, 0.0))
+    T = 1e4
+    o = orc.Oracle(geo, [W.LEAD], phys(33, max_steps_per_track=5), 2, 1)
+    o.begin(W.beam(1, 1, ptype, T), 1)
+    for k in range(1, 5):
+        o.step()
+        st = o.state()[0]
+        assert st["action"] == 4 and st["nsteps"] == k and o.tallies().sum() == 0.0
+    o.step()
+    st = o.state()[0]
+    assert st["action"] == VACANT
+    Tl = o.tallies()[0]
+    assert Tl[0] == 0.0 and abs(Tl[1] - (T + rest)) <= 1e-12 * (T + rest)
+    o.step()                                                                    # nothing left: the run is over
+    assert o.tallies()[0, 1] == Tl[1] and len(o.initializers()) == 0
+
+
+def _walk_photon(o, max_steps=20):
+    """step a single photon in an all-vacuum geometry; returns [(vol, surf, x, y), ...] until it is gone"""
+    out = []
+    for _ in range(max_steps):
+        o.step()
+        st = o.state()[0]
+        if st["action"] == VACANT:
+            out.append(("escaped", float(st["pos"][0]), float(st["pos"][1])))
+            break
+        out.append((int(st["vol"]), int(st["surf"]), float(st["pos"][0]), float(st["pos"][1])))
+    return out
+
+
+def test_cylinder_crossing_sequences():
+    """S6 cylinder crossings: the (vol, surf) transitions a photon goes through in concentric vacuum shells
+    r = 1, 2, 3, 4 cm are fixed by circle-line geometry; written out by hand below (surf = index of the radial
+    boundary the track sits on; crossing outwards vol+1, inwards vol-1)."""
+    geo = dict(kind=1, bounds=np.array([0.0, 1.0, 2.0, 3.0, 4.0]), vol_material=np.full(4, -1, np.int32),
+               vol_bin=np.array([0, 1, 2, 3], np.int32), half_x=0.0, half_y=0.0, half_z=100.0, field=np.zeros(3))
+    o = orc.Oracle(geo, [W.LEAD], phys(34), 1, 1)
+    # radially outwards from the axis
+    o.begin(W.beam(1, 1, W.GAMMA, 1.0, pos=(0, 0, 0), direction=(1, 0, 0)), 1)
+    seq = _walk_photon(o)
+    assert [s[:2] for s in seq[:-1]] == [(1, 1), (2, 2), (3, 3)] and seq[-1][0] == "escaped"
+    assert np.allclose([s[2] for s in seq[:-1]] + [seq[-1][1]], [1.0, 2.0, 3.0, 4.0], rtol=0, atol=1e-12)
+    assert o.tallies()[0, 4] == 1.0 and o.tallies()[0, :4].sum() == 0.0
+    # radially inwards from r = 3.5, through the axis and out on the other side
+    o.begin(W.beam(1, 1, W.GAMMA, 1.0, pos=(3.5, 0, 0), direction=(-1, 0, 0)), 1)
+    seq = _walk_photon(o)
+    assert [s[:2] for s in seq[:-1]] == [(2, 3), (1, 2), (0, 1), (1, 1), (2, 2), (3, 3)] and seq[-1][0] == "escaped"
+    assert np.allclose([s[2] for s in seq[:-1]] + [seq[-1][1]], [3.0, 2.0, 1.0, -1.0, -2.0, -3.0, -4.0], rtol=0, atol=1e-12)
+    # a chord with impact parameter 1.5 cm: reaches shell 1 (1 <= r < 2) but not the core; the line y = 1.5 meets the
+    # circle of radius rho at x = +-sqrt(rho^2 - 2.25)
+    o.begin(W.beam(1, 1, W.GAMMA, 1.0, pos=(-3.5, 1.5, 0), direction=(1, 0, 0)), 1)
+    assert o.locate((-3.5, 1.5, 0.0), (1.0, 0.0, 0.0)) == 3
+    seq = _walk_photon(o)
+    assert [s[:2] for s in seq[:-1]] == [(2, 3), (1, 2), (2, 2), (3, 3)] and seq[-1][0] == "escaped"
+    xs = [-math.sqrt(6.75), -math.sqrt(1.75), math.sqrt(1.75), math.sqrt(6.75), math.sqrt(13.75)]
+    assert np.allclose([s[2] for s in seq[:-1]] + [seq[-1][1]], xs, rtol=0, atol=1e-12)
+    assert all(abs(s[3] - 1.5) < 1e-15 for s in seq[:-1])
+    # a chord with impact parameter 2.5 cm stays in shells 2 and 3
+    o.begin(W.beam(1, 1, W.GAMMA, 1.0, pos=(-3.0, 2.5, 0), direction=(1, 0, 0)), 1)
+    seq = _walk_photon(o)
+    assert [s[:2] for s in seq[:-1]] == [(2, 3), (3, 3)] and seq[-1][0] == "escaped"
+    assert np.allclose([s[2] for s in seq[:-1]] + [seq[-1][1]], [-math.sqrt(2.75), math.sqrt(2.75), math.sqrt(9.75)], rtol=0, atol=1e-12)
+    # the end planes: a photon along z leaves through z = +half_z without any radial crossing
+    o.begin(W.beam(1, 1, W.GAMMA, 1.0, pos=(1.5, 0, 0), direction=(0, 0, 1)), 1)
+    seq = _walk_photon(o)
+    assert len(seq) == 1 and seq[0][0] == "escaped" and o.state()[0]["pos"][2] == 100.0
