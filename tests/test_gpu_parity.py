@@ -180,9 +180,10 @@ def test_shower_lockstep_first_iterations(binding, cfg, sort_mode):
         w = W.config3(n_events=40, n_slots=9000, sort_mode=sort_mode, energy=1e4)
     else:
         w = W.config4(n_events=6, per_event=50, n_slots=9000, sort_mode=sort_mode)
-    agreed = lockstep(binding, w, 60, must_match=5)
+    # floors: what the first GPU run of this test reached (8 / 15-17 / 12-14 iterations) minus a margin; the first
+    # disagreement is checked to be a decision flip of a few slots inside lockstep()
+    agreed = lockstep(binding, w, 60, must_match=5, min_agreed={"calo": 6, "calo_1T": 12, "barrel": 9}[cfg])
     print(f"{cfg} mode {sort_mode}: {agreed} iterations in bit-exact / 1e-12 agreement")
-    assert agreed >= 5
 
 
 def test_positrons_and_annihilation_lockstep(binding):
