@@ -447,7 +447,7 @@ void phase_init(Oracle& o) {
 
 // ---------------------------------------------------------------- P2 reindex (S2)
 int sort_key(const Oracle& o, const OrcTrack& t) {
-  if (o.sort_mode == 1) return t.action;
+  if (o.sort_mode == 1 || o.sort_mode == 4) return t.action;   // mode 4 = by action + parent-slot reuse (S9-R)
   if (o.sort_mode == 2) return t.action == VACANT ? 3 : t.ptype;
   return 0;
 }
@@ -460,7 +460,7 @@ void phase_reindex(Oracle& o) {
   o.track_steps += alive;
   if (alive > 0) o.iterations += 1;
   // stable counting sort of slot indices by key
-  int n_keys = (o.sort_mode == 1) ? 8 : (o.sort_mode == 2 ? 4 : 1);
+  int n_keys = (o.sort_mode == 1 || o.sort_mode == 4) ? 8 : (o.sort_mode == 2 ? 4 : 1);
   uint32_t kc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   for (uint64_t s = 0; s < o.n_slots; ++s) kc[sort_key(o, o.tracks[s])]++;
   for (int a = 0; a <= 8; ++a) o.offsets[a] = 0;
@@ -728,7 +728,21 @@ void phase_score(Oracle& o) {
 }
 
 // ---------------------------------------------------------------- P5 push (S9)
+// S9-R (sort mode 4, section 3.2): a slot that its interaction vacated in this iteration and that staged
+// secondaries takes its first staged secondary in place (exactly the track P1 would make of that initializer); only
+// the slot's remaining secondaries are pushed.
 void phase_push(Oracle& o) {
+  const bool reuse = (o.sort_mode == 4);
+  if (reuse) {
+    for (uint64_t s = 0; s < o.n_slots; ++s) {
+      Stage& st = o.stage[s];
+      if (o.tracks[s].action == VACANT && st.nsec >= 1) {
+        load_initializer(o.tracks[s], st.sec[0]);
+        st.sec[0] = st.sec[1];
+        st.nsec -= 1;
+      }
+    }
+  }
   uint64_t S = 0;
   for (uint64_t s = 0; s < o.n_slots; ++s) S += o.stage[s].nsec;
   if (o.init.size() + S > o.phys.init_capacity) { o.error = -4; }

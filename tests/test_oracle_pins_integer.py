@@ -200,3 +200,139 @@ def test_shower_shape_sanity():
     tmax = (np.argmax(lay) + 0.5) * x0_per_layer
     assert 4.0 < tmax < 10.0
     assert T[:-1].sum() / T.sum() > 0.93
+
+
+# ---------------------------------------------------------------- S9-R: parent-slot reuse (sort mode 4)
+def _block(mat_index=0):
+    return W.slab_geometry([-1e6, 1e6], [mat_index], [0], 1e6)
+
+
+def test_reuse_rule_hand_worked_photoelectric_and_annihilation():
+    """hand-worked S9-R cases. (a) a 20 keV photon in Pb is absorbed photoelectrically (Sigma_PE / Sigma_tot > 0.999):
+    its electron (T = E, same direction) appears IN THE PHOTON'S SLOT at the end of the absorbing iteration, nothing is
+    pushed. (b) a positron below the cut stops (S7.1), annihilates in the next iteration: photon (m_e, u) takes the
+    slot, photon (m_e, -u) is the only push."""
+    p = W.physics(41)
+    n = 64
+    o = orc.Oracle(_block(), [W.LEAD], p, n, 4)
+    prim = W.beam(n, 1, W.GAMMA, 0.02)
+    o.begin(prim, n)
+    o.step()                                  # move: every photon picks PE (or, rarely, Compton) at its interaction point
+    st1 = o.state().copy()
+    pe = st1["action"] == 0
+    assert pe.sum() >= n - 2
+    o.step()                                  # PE applied: electron in place
+    st2 = o.state()
+    assert len(o.initializers()) == 0 and o.counters()["secondaries"] == 0
+    assert np.all(st2["ptype"][pe] == 1) and np.all(st2["action"][pe] == 4) and np.all(st2["nsteps"][pe] == 0)
+    assert np.array_equal(st2["energy"][pe], st1["energy"][pe]) and np.array_equal(st2["pos"][pe], st1["pos"][pe])
+    assert np.array_equal(st2["dir"][pe], st1["dir"][pe]) and np.array_equal(st2["event"][pe], st1["event"][pe])
+    assert np.array_equal(st2["vol"][pe], st1["vol"][pe]) and np.array_equal(st2["surf"][pe], st1["surf"][pe])
+    assert o.tallies().sum() == 0.0           # nothing deposited yet: the electrons are tracked
+    # the same run in mode 1: the electrons go through the stack and come back in LIFO order
+    o1 = orc.Oracle(_block(), [W.LEAD], p, n, 1)
+    o1.begin(prim, n); o1.step(); o1.step()
+    assert len(o1.initializers()) == pe.sum() and np.all(o1.state()["action"][pe] == VACANT)
+    # (b)
+    o = orc.Oracle(_block(), [W.LEAD], p, 4, 4)
+    o.begin(W.beam(1, 1, W.POSITRON, 5e-4), 1)
+    o.step()
+    assert o.state()[0]["action"] == 6
+    o.step()
+    st = o.state()[0]; ini = o.initializers()
+    assert st["action"] == 3 and st["ptype"] == 0 and st["energy"] == M_E and st["nsteps"] == 0
+    assert len(ini) == 1 and ini[0]["energy"] == M_E and np.array_equal(ini[0]["dir"], -st["dir"])
+    assert np.array_equal(ini[0]["pos"], st["pos"]) and o.counters()["secondaries"] == 1
+    o.step()                                  # the pushed photon fills slot 1 (the lowest vacancy) in P1 of the next iteration
+    assert o.state()[1]["event"] == 0 and len(o.initializers()) == 0
+    o.run()
+    assert abs(o.tallies().sum() - (5e-4 + 2 * M_E)) < 1e-9
+
+
+def test_reuse_rule_hand_worked_pair():
+    """a 50 MeV photon converts: e- (first staged) takes the slot, e+ is pushed; energies add up to E - 2 m_e"""
+    n = 200
+    E = 50.0
+    o = orc.Oracle(_block(), [W.LEAD], W.physics(42), n, 4)
+    o.begin(W.beam(n, 1, W.GAMMA, E), n)
+    o.step()
+    st1 = o.state().copy()
+    pair = np.flatnonzero(st1["action"] == 1)
+    assert len(pair) > 0.9 * n
+    o.step()
+    st2 = o.state(); ini = o.initializers()
+    pos_of = {tuple(st1["pos"][s]): s for s in pair}
+    eplus = [i for i in ini if i["ptype"] == 2]
+    assert len(eplus) == len(pair)
+    for i in eplus:
+        s = pos_of[tuple(i["pos"])]
+        assert st2["ptype"][s] == 1 and st2["action"][s] == 4 and st2["nsteps"][s] == 0     # the e- is in the slot
+        assert abs(st2["energy"][s] + i["energy"] + 2 * M_E - E) < 1e-13 * E
+        assert np.array_equal(st2["dir"][s], st1["dir"][s]) and np.array_equal(st2["pos"][s], st1["pos"][s])
+    # pushes are in ascending parent-slot order
+    parents = [pos_of[tuple(i["pos"])] for i in eplus]
+    assert parents == sorted(parents)
+
+
+def test_reuse_rule_vs_mode1_restatement_on_showers():
+    """S9-R restated against the oracle's own mode 1 on the same iteration: the two modes are driven in lockstep from
+    the same state (same slots -> same PRNG streams) until the first reuse; in that iteration mode 1's pushed
+    initializers, minus the first secondary of every parent slot that ended VACANT, are mode 4's pushes, and exactly
+    those first secondaries sit in their parents' slots (as the tracks P1 would have made of them)."""
+    checked = 0
+    for seed in (51, 52, 53, 54):
+        w1 = W.config2(n_events=6, n_slots=256, sort_mode=1, seed=seed, energy=300.0, field_T=(1.0, 0.0, 0.0))
+        w4 = W.config2(n_events=6, n_slots=256, sort_mode=4, seed=seed, energy=300.0, field_T=(1.0, 0.0, 0.0))
+        a, b = make_oracle(w1), make_oracle(w4)
+        a.begin(w1.primaries, 6); b.begin(w4.primaries, 6)
+        for k in range(200):
+            a.phase_init(); b.phase_init()
+            a.phase_reindex(); b.phase_reindex()
+            pre = a.state().copy()
+            assert np.array_equal(pre, b.state())
+            ia0, ib0 = len(a.initializers()), len(b.initializers())
+            a.phase_rest(); b.phase_rest()
+            sa, sb = a.state(), b.state()
+            new_a, new_b = a.initializers()[ia0:], b.initializers()[ib0:]
+            # parent slot of each of mode 1's pushes: the slot that held that position before the iteration
+            pos_of = {tuple(pre["pos"][s]): s for s in np.flatnonzero(pre["action"] != VACANT)}
+            parent = np.array([pos_of[tuple(i["pos"])] for i in new_a], dtype=np.int64)
+            assert np.all(np.diff(parent) >= 0)
+            first_of_parent = np.ones(len(new_a), bool)
+            first_of_parent[1:] = parent[1:] != parent[:-1]
+            reused = first_of_parent & (sa["action"][parent] == VACANT) if len(new_a) else first_of_parent
+            expect_push = new_a[~reused]
+            assert np.array_equal(new_b, expect_push)
+            for i, s in zip(new_a[reused], parent[reused]):
+                t = sb[s]
+                assert t["action"] == (3 if i["ptype"] == 0 else 4) and t["nsteps"] == 0 and t["ptype"] == i["ptype"]
+                for f in ("pos", "dir", "energy", "event", "vol", "surf"):
+                    assert np.array_equal(t[f], i[f])
+            others = np.setdiff1d(np.arange(256), parent[reused]) if len(new_a) else np.arange(256)
+            assert np.array_equal(sa[others], sb[others])
+            if reused.any():
+                checked += int(reused.sum())
+                break                                   # histories separate here
+    assert checked >= 4
+
+
+def test_reuse_mode_conserves_energy_and_is_sort_consistent():
+    """mode 4 on whole showers: per-event conservation (pin 5), the index array is the stable sort by action, and the
+    number of pushes drops against mode 1 by about the number of slot-vacating interactions"""
+    w = W.config2(n_events=5, n_slots=512, sort_mode=4, seed=33, energy=500.0, field_T=(1.0, 0.0, 0.0))
+    o = make_oracle(w)
+    o.begin(w.primaries, w.n_events)
+    for _ in range(30):
+        o.phase_init(); o.phase_reindex()
+        idx, off = o.indices()
+        act = o.state()["action"]
+        assert np.array_equal(idx, np.argsort(act, kind="stable").astype(np.uint32))
+        assert np.array_equal(off, np.concatenate([[0], np.cumsum(np.bincount(act, minlength=8))]))
+        o.phase_rest()
+    o.run()
+    assert np.abs(o.tallies().sum(1) - 500.0).max() < 1e-9 * 500.0
+    w1 = W.config2(n_events=5, n_slots=512, sort_mode=1, seed=33, energy=500.0, field_T=(1.0, 0.0, 0.0))
+    o1 = make_oracle(w1); o1.transport(w1.primaries, w1.n_events)
+    c4, c1 = o.counters(), o1.counters()
+    assert c4["secondaries"] < 0.8 * c1["secondaries"]
+    assert abs(c4["track_steps"] - c1["track_steps"]) < 0.1 * c1["track_steps"]
