@@ -29,7 +29,7 @@ if ROOT not in sys.path:
 
 from paper_2503_17608_b200 import workloads as W  # noqa: E402  (input data only)
 
-SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle", 3: "partition"}
+SORT_NAMES = {0: "none", 1: "by_action", 2: "by_particle", 3: "partition", 4: "by_action_reuse"}
 ACTIONS = ("PE", "PAIR", "COMPTON", "MOVE_G", "MOVE_C", "BREMS", "ANNIH", "VACANT")
 STATE_BYTES = 64          # one slot's state: RecA + RecB
 INDEX_BYTES = 4
@@ -175,7 +175,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     counts: [iterations][8] action counts after P1. Returns {kernel name: bytes}."""
     c = counts.astype(np.float64).sum(0)
     it = float(len(counts))
-    idx = INDEX_BYTES if sort_mode in (1, 2) else 0
+    idx = INDEX_BYTES if sort_mode in (1, 2, 4) else 0
     rw = 2 * STATE_BYTES + idx          # gather + write back one slot through the index
     n = float(n_slots)
     sec = float(n_secondaries)
@@ -350,7 +350,7 @@ def run_cuda(args):
     # ---- the other sort modes (BASELINE.json metric: per sort mode)
     per_mode = {}
     if not args.no_modes:
-        for mode in (0, 1, 2, 3):
+        for mode in (0, 1, 2, 3, 4):
             if mode == w.sort_mode:
                 per_mode[SORT_NAMES[mode]] = {"track_steps_per_s": track_steps / (ms * 1e-3) / world if world > 1 else track_steps / (ms * 1e-3),
                                               "events_per_s": w.n_events * args.steps / (ms * 1e-3)}
@@ -404,7 +404,7 @@ def main():
     ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4", "config5"])
     ap.add_argument("--events", type=int, default=0, help="override the workload's number of events")
     ap.add_argument("--slots", type=int, default=0, help="override the workload's number of track slots")
-    ap.add_argument("--sort-mode", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--sort-mode", type=int, default=1, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--no-modes", action="store_true", help="skip the other sort modes")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--oracle-events", type=int, default=200, help="events in the oracle's bounded sample")

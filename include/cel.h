@@ -28,7 +28,11 @@ enum { CEL_SORT_NONE = 0, CEL_SORT_BY_ACTION = 1, CEL_SORT_BY_PARTICLE = 2,
        /* PAPER.md:51 (section 3.2): no index array; the initializers popped in an iteration are partitioned by charge and
         * assigned to opposite ends of the track array (docs/PHYSICS_SPEC.md S9-P): charged ones take the vacancies from
         * slot 0 upwards, neutral ones from slot N-1 downwards; the kernels run masked over all slots as in mode NONE */
-       CEL_SORT_PARTITION = 3 };
+       CEL_SORT_PARTITION = 3,
+       /* PAPER.md:53 (section 3.2): reindexing by action as CEL_SORT_BY_ACTION, plus parent-slot reuse (S9-R): a slot
+        * vacated by its interaction (photoelectric, pair, annihilation, a Compton photon / bremsstrahlung electron that fell
+        * below the cut) takes the interaction's first secondary in place instead of pushing it to the initializer stack */
+       CEL_SORT_BY_ACTION_REUSE = 4 };
 enum { CEL_GEOM_SLAB = 0, CEL_GEOM_CYL = 1 };
 enum { CEL_GAMMA = 0, CEL_ELECTRON = 1, CEL_POSITRON = 2 };
 /* action IDs = sort keys (docs/PHYSICS_SPEC.md S2) */

@@ -250,7 +250,7 @@ extern "C" uint64_t cel_workspace_bytes(uint64_t n_slots, uint64_t init_capacity
 extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n_mats, const cel_physics* ph,
                           uint64_t n_slots, int sort_mode, cel_ctx** out) {
   if (!g || !mats || !ph || !out || n_mats < 1 || n_slots < 1 || n_slots > (1ull << 31)) return CEL_ERR_INVALID_ARG;
-  if (sort_mode < 0 || sort_mode > CEL_SORT_PARTITION || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
+  if (sort_mode < 0 || sort_mode > CEL_SORT_BY_ACTION_REUSE || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
   if (g->n_vol < 1 || g->n_vol > 254 || !g->bounds || !g->vol_material || !g->vol_bin) return CEL_ERR_INVALID_ARG;
   for (int i = 0; i < g->n_vol; ++i) {
     if (!(g->bounds[i] < g->bounds[i + 1])) return CEL_ERR_INVALID_ARG;
@@ -327,7 +327,8 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   P.energy_nodes = (const double*)(db + o_en);
   const Tiling tl = make_tiling(n_slots);
   D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
-  D.sort_mode = sort_mode;
+  D.sort_mode = sort_mode == CEL_SORT_BY_ACTION_REUSE ? CEL_SORT_BY_ACTION : sort_mode;   // the index sort is the same;
+  D.reuse = sort_mode == CEL_SORT_BY_ACTION_REUSE ? 1 : 0;                               // only the interaction epilogues differ (S9-R)
   D.init_capacity = default_capacity(n_slots, ph->init_capacity);
 
   if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(CEL_ERR_CUDA);

@@ -128,7 +128,8 @@ struct DeviceState {
   uint32_t n_tiles;
   uint32_t tile_shift;    // log2(tile_slots)
   uint32_t subs_per_tile; // tile_slots / kSub
-  int sort_mode;
+  int sort_mode;          // 0 none, 1 by action, 2 by particle, 3 partition (CEL_SORT_BY_ACTION_REUSE is 1 here, with reuse = 1)
+  int reuse;              // S9-R: a slot vacated by its interaction takes its first secondary in place
   int write_vacant;       // 1 = also write the indices of vacant slots (complete permutation, debug surface)
   unsigned long long init_capacity;
   uint32_t n_events;

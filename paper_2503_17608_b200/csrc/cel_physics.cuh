@@ -74,6 +74,13 @@ __device__ __forceinline__ void stage_secondary(const DeviceState& D, uint32_t s
   store_b(D.secB + 2ull * slot + j, b);
 }
 
+// S9-R (sort mode 4): the slot its interaction vacates takes the interaction's first secondary in place —
+// the track P1 would have made of that initializer (parent's event, position, vol, surf; nsteps = 0). Returns its action.
+__device__ __forceinline__ int become_secondary(Track& t, double energy, double dx, double dy, double dz, int ptype) {
+  t.a.energy = energy; t.dx = dx; t.dy = dy; t.dz = dz; t.ptype = ptype; t.nsteps = 0;
+  return ptype == P_GAMMA ? A_MOVE_G : A_MOVE_C;
+}
+
 // a charged track whose kinetic energy dropped below the cut (its energy is already in edep): returns the new action
 __device__ __forceinline__ int stop_charged(const Params& P, int ptype, double& edep) {
   if (ptype == P_POSITRON) {
@@ -129,10 +136,11 @@ __device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) 
 __device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t slot, const RecA& a, const RecB& b) {
   Track t = unpack(a, b);
   double edep = 0.0;
-  int nsec = 0;
+  int nsec = 0, action = A_VACANT;
   if (D.P.electrons_local) edep += t.a.energy;
+  else if (D.reuse) action = become_secondary(t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);   // only the meta word changes
   else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
-  finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+  finish(D, slot, t, action, t.vol, edep, 0.0, nsec, false);
 }
 template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
@@ -157,6 +165,13 @@ __device__ __forceinline__ void do_pair(const DeviceState& D, uint32_t slot, uin
   const double Tav = t.a.energy - 2.0 * kElectronMass;
   const double Tm = xi0 * Tav;
   const double Tp = Tav - Tm;
+  if (D.reuse) {   // S9-R: the first staged secondary (e-, or e+ when the e- is below the cut) takes the slot
+    int action;
+    if (Tm >= P.cut) { stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON); action = become_secondary(t, Tm, t.dx, t.dy, t.dz, P_ELECTRON); }
+    else { edep += Tm; action = become_secondary(t, Tp, t.dx, t.dy, t.dz, P_POSITRON); }
+    finish(D, slot, t, action, t.vol, edep, 0.0, nsec, true);
+    return;
+  }
   if (Tm >= P.cut) stage_secondary(D, slot, nsec++, t, Tm, t.dx, t.dy, t.dz, P_ELECTRON);
   else edep += Tm;
   stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
@@ -184,6 +199,12 @@ __device__ __forceinline__ void do_annihilation(const DeviceState& D, uint32_t s
   double sp, cp;
   sincospi(2.0 * xi1, &sp, &cp);
   const double ux = sint * cp, uy = sint * sp, uz = cost;
+  if (D.reuse) {   // S9-R: photon (m_e, u) takes the slot, photon (m_e, -u) is pushed
+    stage_secondary(D, slot, 0, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
+    const int action = become_secondary(t, kElectronMass, ux, uy, uz, P_GAMMA);
+    finish(D, slot, t, action, t.vol, 0.0, 0.0, 1, true);
+    return;
+  }
   stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
   stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
   finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
@@ -201,8 +222,9 @@ __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
 }
 
 // ================================================================ photons: Compton (S8) then move (S5)
-// S8 Compton: Klein-Nishina epsilon-mixture rejection; returns false if the photon fell below the cut (absorbed)
-__device__ __forceinline__ bool compton(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, int& nsec) {
+// S8 Compton: Klein-Nishina epsilon-mixture rejection; returns the slot's action: MOVE_G (the photon goes on and moves
+// in this iteration), VACANT (it fell below the cut), or MOVE_C (S9-R: it fell below the cut and its electron took the slot)
+__device__ __forceinline__ int compton(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, int& nsec) {
   const Params& P = D.P;
   const double E = t.a.energy;
   const double k = E / kElectronMass;
@@ -232,11 +254,12 @@ __device__ __forceinline__ bool compton(const DeviceState& D, uint32_t slot, uin
     double ex = E * t.dx - E1 * d1x, ey = E * t.dy - E1 * d1y, ez = E * t.dz - E1 * d1z;
     const double n = sqrt(ex * ex + ey * ey + ez * ez);
     if (n > 0.0) { ex /= n; ey /= n; ez /= n; } else { ex = t.dx; ey = t.dy; ez = t.dz; }
+    if (D.reuse && E1 < P.cut) { edep += E1; return become_secondary(t, Te, ex, ey, ez, P_ELECTRON); }
     stage_secondary(D, slot, nsec++, t, Te, ex, ey, ez, P_ELECTRON);
   }
-  if (E1 < P.cut) { edep += E1; return false; }
+  if (E1 < P.cut) { edep += E1; return A_VACANT; }
   t.a.energy = E1; t.dx = d1x; t.dy = d1y; t.dz = d1z;
-  return true;
+  return A_MOVE_G;
 }
 
 // S5 photon move: sampled free path vs distance to boundary; returns the next action
@@ -285,10 +308,9 @@ __device__ __forceinline__ void do_photon(const DeviceState& D, uint32_t slot, u
   const int vol0 = t.vol;
   double edep = 0.0, eesc = 0.0;
   int nsec = 0;
-  int action = A_VACANT;
-  bool alive = true;
-  if (act == A_COMPTON) alive = compton(D, slot, k_iter, t, edep, nsec);
-  if (alive) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
+  int action = A_MOVE_G;
+  if (act == A_COMPTON) action = compton(D, slot, k_iter, t, edep, nsec);
+  if (action == A_MOVE_G) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
   finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
 }
 // (four blocks per SM = 64 registers: measured 1-3 % faster than the 80 the compiler takes unasked)
@@ -451,16 +473,23 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
     double xi0, xi1;
     draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
     const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
-    stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
     const double T1 = t.a.energy - kph;
-    if (T1 < P.cut) { edep += T1; t.a.energy = 0.0; action = stop_charged(P, t.ptype, edep); }
-    else t.a.energy = T1;
+    if (T1 < P.cut) {
+      edep += T1;
+      action = stop_charged(P, t.ptype, edep);
+      if (D.reuse && action == A_VACANT) action = become_secondary(t, kph, t.dx, t.dy, t.dz, P_GAMMA);   // S9-R: the photon takes the slot
+      else { stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA); t.a.energy = 0.0; }
+    } else {
+      stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
+      t.a.energy = T1;
+    }
   }
   if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
   finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
 }
+// (without a field: four blocks per SM = 64 registers, the count the kernel is tuned at — 70+ registers measured 19 % slower)
 template <bool FIELD, int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock) k_charged(DeviceState D) {
+__global__ void __launch_bounds__(kBlock, FIELD ? 2 : 4) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }

@@ -16,7 +16,7 @@ import numpy as np
 
 PRIMARY_DTYPE = np.dtype([("event", "<u4"), ("ptype", "<i4"), ("energy", "<f8"), ("pos", "<f8", 3), ("dir", "<f8", 3)])
 GAMMA, ELECTRON, POSITRON = 0, 1, 2
-SORT_NONE, SORT_BY_ACTION, SORT_BY_PARTICLE, SORT_PARTITION = 0, 1, 2, 3
+SORT_NONE, SORT_BY_ACTION, SORT_BY_PARTICLE, SORT_PARTITION, SORT_BY_ACTION_REUSE = 0, 1, 2, 3, 4
 
 LEAD = (11.35, 82.0, 207.2)
 LAR = (1.396, 18.0, 39.95)
