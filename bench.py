@@ -180,8 +180,9 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     n = float(n_slots)
     sec = float(n_secondaries)
     out = {
-        "init_fill": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES,   # key bytes + (read init, write slot)
-        "scatter": it * n * 1 + (it * n - c[7]) * idx,                      # key bytes + one index per non-vacant slot
+        # key bytes read once (an upper bound: tiles that are entirely vacant and get no fill are skipped) + (read init,
+        # write slot) per initialised track + one index per non-vacant slot
+        "fill_sort": it * n * 1 + float(n_initialised) * 2 * STATE_BYTES + (it * n - c[7]) * idx,
         "annihilation": c[6] * (rw + 2 * STATE_BYTES),
         "photoelectric": c[0] * (rw + STATE_BYTES),
         "pair": c[1] * (rw + 2 * STATE_BYTES),
@@ -193,7 +194,7 @@ def algorithmic_bytes(counts, n_slots, sort_mode, n_initialised, n_secondaries):
     out["part_count"] = float(n_initialised) * 8
     out["part_scatter"] = float(n_initialised) * (8 + INDEX_BYTES)
     if sort_mode == 3:
-        out["init_fill"] += float(n_initialised) * INDEX_BYTES
+        out["fill_sort"] += float(n_initialised) * INDEX_BYTES
     out["discrete"] = sum(out[k] for k in ("annihilation", "photoelectric", "pair"))
     return out
 

@@ -48,7 +48,9 @@ enum {
   CEL_ERR_TALLY_OVERFLOW = -5,
   CEL_ERR_NONFINITE = -6,     /* a non-finite energy or position was produced */
   CEL_ERR_NOT_RUN = -7,       /* cel_tallies before any cel_transport */
-  CEL_ERR_MAX_ITER = -8       /* the run did not end within max_iterations */
+  CEL_ERR_MAX_ITER = -8,      /* the run did not end within max_iterations */
+  CEL_ERR_INTERNAL = -9       /* a bookkeeping block gave up waiting for the blocks before it (cannot happen when blocks
+                                 are dispatched in index order; reported instead of hanging) */
 };
 
 /* one effective element per material (S0) */
@@ -94,7 +96,7 @@ typedef struct {
 } cel_tally_view;
 
 /* Create a context: builds the physics tables on the host (S4), uploads geometry and tables, allocates the
- * SoA state for n_slots slots (N <= 2^31), the staging areas and the initializer stack. mats: n_mats entries.
+ * SoA state for n_slots slots (N <= 2^28), the staging areas and the initializer stack. mats: n_mats entries.
  * sort_mode: CEL_SORT_*. On success *out owns device memory until cel_destroy. */
 int cel_create(const cel_geometry* geometry, const cel_material* mats, int n_mats, const cel_physics* physics,
                uint64_t n_slots, int sort_mode, cel_ctx** out);
@@ -126,10 +128,10 @@ void cel_destroy(cel_ctx*);
 const char* cel_strerror(int code);
 const char* cel_last_cuda_error(cel_ctx*);
 
-/* The kernels of one step iteration (S1). P1 (+ the P2 histogram): INIT_FILL; P2: SCATTER (sorted modes);
+/* The kernels of one step iteration (S1). P1 + P2 + the iteration's counters: FILL_SORT (one pass);
  * P3i: ANNIH, PE, PAIR; P3i+P3m: PHOTON (Compton, then the photon move), CHARGED (bremsstrahlung, then the charged move
  * with energy loss and MSC); P4 (scoring) happens inside the action kernels; P5: PUSH. */
-enum { CEL_K_INIT_FILL = 0, CEL_K_SCATTER, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
+enum { CEL_K_FILL_SORT = 0, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
        CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
        CEL_K_DISCRETE /* photoelectric + pair + annihilation in one launch (sort by action, option merge_discrete) */,
        CEL_KERNEL_COUNT };

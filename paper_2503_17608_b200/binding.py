@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libcelstep.so")
+LIB_PATH = os.environ.get("CELSTEP_LIB") or os.path.join(HERE, "libcelstep.so")   # (CELSTEP_LIB: another build of the same ABI, for A/B timing)
 
 PRIMARY_DTYPE = np.dtype([("event", "<u4"), ("ptype", "<i4"), ("energy", "<f8"), ("pos", "<f8", 3), ("dir", "<f8", 3)])
 TRACK_DTYPE = np.dtype([("pos", "<f8", 3), ("dir", "<f8", 3), ("energy", "<f8"), ("event", "<u4"),

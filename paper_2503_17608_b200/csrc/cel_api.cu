@@ -16,7 +16,7 @@ using namespace cel;
 
 static_assert(sizeof(cel_primary) == 64 && sizeof(PrimaryRec) == 64, "cel_primary layout");
 static_assert(sizeof(cel_track) == 80 && sizeof(TrackRec) == 80, "cel_track layout");
-static_assert((int)K_COUNT == (int)CEL_KERNEL_COUNT && (int)K_PUSH == (int)CEL_K_PUSH && (int)K_CHARGED == (int)CEL_K_CHARGED, "kernel ids");
+static_assert((int)K_COUNT == (int)CEL_KERNEL_COUNT && (int)K_PUSH == (int)CEL_K_PUSH && (int)K_CHARGED == (int)CEL_K_CHARGED && (int)K_FILL_SORT == (int)CEL_K_FILL_SORT, "kernel ids");
 static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32, "record layout");
 static_assert(sizeof(DeviceState) < 3500, "DeviceState must fit in kernel parameter space");
 
@@ -25,6 +25,7 @@ namespace {
 constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action counts are logged
 constexpr int kStatusSlots = 2;
 constexpr int kMaxKernelsPerIteration = 16;
+static_assert(CEL_ERR_INTERNAL == -9, "k_fill_sort sets -9");
 constexpr int kSideStreams = 4;
 
 struct HostTables {                 // per material, kept for cel_debug_table
@@ -42,6 +43,7 @@ struct cel_ctx {
   cel_geometry geo{};
   std::vector<double> h_bounds; std::vector<int> h_vol_material, h_vol_bin;
   uint64_t n_slots = 0;
+  int user_sort_mode = 0;           // the CEL_SORT_* value given to cel_create (D.sort_mode folds BY_ACTION_REUSE into BY_ACTION)
   // device-resident read-only data (small)
   void* d_params_blob = nullptr;
   // workspace
@@ -174,20 +176,31 @@ struct Layout {
   uint64_t stA, stB, akey, nsec, indices, secA, secB, initA, initB, ctl, log, total;
 };
 
-// bookkeeping tiles (cel_device.cuh): sub-tiles of kSub slots, at most kMaxTiles tiles of 2^shift slots
-struct Tiling { uint32_t n_tiles, tile_shift, subs_per_tile; };
-Tiling make_tiling(uint64_t N) {
+// bookkeeping tiles (cel_device.cuh): sub-tiles of kSub slots, tiles of 2^shift slots in groups of kGroupTiles
+struct Tiling { uint32_t n_tiles, tile_shift, subs_per_tile, n_groups; };
+uint64_t g_max_tiles_small = 2048, g_max_tiles_large = 4096;   // (cel_set_option "max_tiles": measurement knob)
+Tiling make_tiling(uint64_t N, uint64_t max_tiles_override = 0) {
   const uint64_t subs = (N + kSub - 1) / kSub;
   uint32_t spt = 1, shift = 10;
   static_assert(kSub == 1024, "tile_shift assumes 1024-slot sub-tiles");
-  // at most 2048 tiles up to 2^22 slots, kMaxTiles = 4096 beyond (measured: more, smaller tiles pay only when a block
-  // would otherwise walk 8 sub-tiles; at 2^22 slots 4096 blocks per bookkeeping kernel raise the per-iteration floor)
-  const uint64_t max_tiles = N > (1ull << 22) ? (uint64_t)kMaxTiles : 2048ull;
+  // at most 2048 tiles up to 2^22 slots, 4096 beyond (measured: more, smaller tiles pay only when a block would
+  // otherwise walk many sub-tiles; every block of a bookkeeping kernel costs launch time in the lightly loaded iterations)
+  uint64_t max_tiles = N > (1ull << 22) ? g_max_tiles_large : g_max_tiles_small;
+  if (max_tiles_override) max_tiles = max_tiles_override;
+  if (max_tiles > (uint64_t)kMaxTiles) max_tiles = kMaxTiles;
   while ((subs + spt - 1) / spt > max_tiles) { spt *= 2; shift += 1; }
   Tiling t;
   t.subs_per_tile = spt; t.tile_shift = shift;
   t.n_tiles = (uint32_t)((N + ((uint64_t)1 << shift) - 1) >> shift);
+  t.n_groups = (t.n_tiles + kGroupTiles - 1) / kGroupTiles;
   return t;
+}
+
+int n_index_regions(int sort_mode) {   // regions of N entries in the index array (cel_device.cuh: DeviceState::indices)
+  if (sort_mode == CEL_SORT_BY_ACTION || sort_mode == CEL_SORT_BY_ACTION_REUSE) return 8;
+  if (sort_mode == CEL_SORT_BY_PARTICLE) return 4;
+  if (sort_mode == CEL_SORT_PARTITION) return 1;   // plist
+  return 0;
 }
 
 Layout make_layout(uint64_t N, uint64_t cap, int sort_mode) {
@@ -200,7 +213,7 @@ Layout make_layout(uint64_t N, uint64_t cap, int sort_mode) {
   L.stB = take(N * sizeof(RecB));
   L.akey = take(padded);
   L.nsec = take(padded);
-  L.indices = take(sort_mode != CEL_SORT_NONE ? N * sizeof(uint32_t) : 0);
+  L.indices = take((uint64_t)n_index_regions(sort_mode) * N * sizeof(uint32_t));
   L.secA = take(2 * N * sizeof(RecA));
   L.secB = take(2 * N * sizeof(RecB));
   L.initA = take(cap * sizeof(RecA));
@@ -219,7 +232,7 @@ uint64_t default_capacity(uint64_t N, uint64_t cap) {
 
 int lay_out(cel_ctx* c) {
   if (c->laid_out) return CEL_OK;
-  const Layout L = make_layout(c->n_slots, c->D.init_capacity, c->D.sort_mode);
+  const Layout L = make_layout(c->n_slots, c->D.init_capacity, c->user_sort_mode);
   if (!c->workspace) {
     CEL_CUDA(c, cudaMalloc(&c->workspace, L.total));
     c->workspace_bytes = L.total; c->own_workspace = true;
@@ -230,7 +243,7 @@ int lay_out(cel_ctx* c) {
   DeviceState& D = c->D;
   D.stA = (RecA*)(base + L.stA); D.stB = (RecB*)(base + L.stB);
   D.akey = (uint8_t*)(base + L.akey); D.nsec = (uint8_t*)(base + L.nsec);
-  D.indices = (D.sort_mode != CEL_SORT_NONE) ? (uint32_t*)(base + L.indices) : nullptr;
+  D.indices = n_index_regions(c->user_sort_mode) ? (uint32_t*)(base + L.indices) : nullptr;
   D.secA = (RecA*)(base + L.secA); D.secB = (RecB*)(base + L.secB);
   D.initA = (RecA*)(base + L.initA); D.initB = (RecB*)(base + L.initB);
   D.ctl = (Control*)(base + L.ctl);
@@ -249,7 +262,7 @@ extern "C" uint64_t cel_workspace_bytes(uint64_t n_slots, uint64_t init_capacity
 // ================================================================ create / destroy
 extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n_mats, const cel_physics* ph,
                           uint64_t n_slots, int sort_mode, cel_ctx** out) {
-  if (!g || !mats || !ph || !out || n_mats < 1 || n_slots < 1 || n_slots > (1ull << 31)) return CEL_ERR_INVALID_ARG;
+  if (!g || !mats || !ph || !out || n_mats < 1 || n_slots < 1 || n_slots > (1ull << 28)) return CEL_ERR_INVALID_ARG;
   if (sort_mode < 0 || sort_mode > CEL_SORT_BY_ACTION_REUSE || (g->kind != CEL_GEOM_SLAB && g->kind != CEL_GEOM_CYL)) return CEL_ERR_INVALID_ARG;
   if (g->n_vol < 1 || g->n_vol > 254 || !g->bounds || !g->vol_material || !g->vol_bin) return CEL_ERR_INVALID_ARG;
   for (int i = 0; i < g->n_vol; ++i) {
@@ -326,7 +339,8 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   P.charged_xs = (const ChargedXs*)(db + o_ch); P.range_tab = (const double*)(db + o_rg);
   P.energy_nodes = (const double*)(db + o_en);
   const Tiling tl = make_tiling(n_slots);
-  D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
+  D.N = (uint32_t)n_slots; D.n_tiles = tl.n_tiles; D.n_groups = tl.n_groups; D.tile_shift = tl.tile_shift; D.subs_per_tile = tl.subs_per_tile;
+  c->user_sort_mode = sort_mode;
   D.sort_mode = sort_mode == CEL_SORT_BY_ACTION_REUSE ? CEL_SORT_BY_ACTION : sort_mode;   // the index sort is the same;
   D.reuse = sort_mode == CEL_SORT_BY_ACTION_REUSE ? 1 : 0;                               // only the interaction epilogues differ (S9-R)
   D.init_capacity = default_capacity(n_slots, ph->init_capacity);
@@ -384,7 +398,7 @@ extern "C" int cel_set_stream(cel_ctx* c, void* s) {
 
 extern "C" int cel_set_workspace(cel_ctx* c, void* dptr, uint64_t bytes) {
   if (!c || !dptr || c->laid_out || ((uintptr_t)dptr & 255)) return CEL_ERR_INVALID_ARG;
-  if (bytes < make_layout(c->n_slots, c->D.init_capacity, c->D.sort_mode).total) return CEL_ERR_INVALID_ARG;
+  if (bytes < make_layout(c->n_slots, c->D.init_capacity, c->user_sort_mode).total) return CEL_ERR_INVALID_ARG;
   c->workspace = dptr; c->workspace_bytes = bytes; c->own_workspace = false;
   return CEL_OK;
 }
@@ -415,6 +429,7 @@ extern "C" const char* cel_strerror(int code) {
     case CEL_ERR_NONFINITE: return "non-finite track state";
     case CEL_ERR_NOT_RUN: return "no transport has run";
     case CEL_ERR_MAX_ITER: return "iteration limit reached";
+    case CEL_ERR_INTERNAL: return "internal error: a bookkeeping wait gave up";
     default: return "unknown error";
   }
 }
@@ -430,7 +445,7 @@ int physics_grid(const cel_ctx* c) {
 }
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
-    "init_fill", "scatter", "annihilation", "photoelectric", "pair", "photon", "charged", "push",
+    "fill_sort", "annihilation", "photoelectric", "pair", "photon", "charged", "push",
     "part_count", "part_scatter", "discrete"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
@@ -470,11 +485,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     launch_chain(c, k_part_count<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_COUNT, n);
     launch_chain(c, k_part_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PART_SCATTER, n);
   }
-  const bool many_tiles = D.n_tiles > 2048u;   // 16 instead of 8 tile counters per thread in the block prefix
-  if (many_tiles) launch_chain(c, k_init_fill<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_init_fill<TR, 8>, tg, kTileThreads, s);
-  after_launch(c, CEL_K_INIT_FILL, n);
-  // (every sort mode: besides the index scatter of the sorted modes it closes the fill — vacancy counters, control block)
-  launch_chain(c, k_scatter<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_SCATTER, n);
+  launch_chain(c, k_fill_sort<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_FILL_SORT, n);   // P1 + P2 + S11 in one pass
   const bool fork = c->concurrent && !c->profile;
   const bool by_action = D.sort_mode == CEL_SORT_BY_ACTION;
   if ((D.sort_mode == CEL_SORT_NONE || D.sort_mode == CEL_SORT_PARTITION) && c->merge_discrete) {
@@ -489,7 +500,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     else { if (field) k_charged<true, 0, TR><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0, TR><<<pg, kBlock, 0, s>>>(D); }
     after_launch(c, CEL_K_CHARGED, n);
     if (fork) { cudaEventRecord(c->ev_join[0], c->side[0]); cudaStreamWaitEvent(s, c->ev_join[0], 0); }
-    if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
     return n;
   }
   // sorted by action: photon, annihilation, photoelectric, pair on one branch each (their ranges are disjoint and fixed);
@@ -521,7 +532,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     cudaEventRecord(c->ev_join[i], c->side[i]);
     cudaStreamWaitEvent(s, c->ev_join[i], 0);
   }
-  if (many_tiles) launch_chain(c, k_push<TR, 16>, tg, kTileThreads, s); else launch_chain(c, k_push<TR, 8>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+  launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
   return n;
 }
 int enqueue_iteration(cel_ctx* c) { return c->trace_iters > 0 ? enqueue_iteration_t<true>(c) : enqueue_iteration_t<false>(c); }
@@ -551,24 +562,19 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   if (c->scratch) { CEL_CUDA(c, cudaFreeAsync(c->scratch, s)); c->scratch = nullptr; }
   if (c->d_tally) { CEL_CUDA(c, cudaFreeAsync(c->d_tally, s)); c->d_tally = nullptr; }
   const uint64_t tiles = D.n_tiles;
-  const uint64_t o_vac = 0, o_sec = align_up(tiles * 4, 256), o_hist = align_up(o_sec + tiles * 4, 256);
-  const uint64_t o_phist = align_up(o_hist + tiles * 32, 256);
-  const uint64_t o_part = align_up(o_phist + tiles * 32, 256);
-  const uint64_t o_filled = align_up(o_part + tiles * 4, 256);
-  const uint64_t o_group = align_up(o_filled + tiles * 4, 256);
-  const uint64_t group_bytes = 2ull * kMaxGroups * 8 * sizeof(uint32_t);
-  const uint64_t scratch_bytes = align_up(o_group + 2 * group_bytes, 256);
+  uint64_t so = 0;
+  auto stake = [&](uint64_t bytes) { uint64_t r = so; so = align_up(so + bytes, 256); return r; };
+  const uint64_t o_vac = stake(2 * tiles * 4), o_sec = stake(tiles * 4);
+  const uint64_t o_hist = stake(tiles * 32), o_phist = stake(tiles * 16), o_rows = stake(2ull * kMaxGroups * kRowWords * 4);
+  const uint64_t o_gmask = stake(2ull * (kMaxGroups / 32) * 4), o_part = stake(tiles * 4);
+  const uint64_t scratch_bytes = so;
   CEL_CUDA(c, cudaMallocAsync(&c->scratch, scratch_bytes, s));
   const uint64_t tally_bytes = (uint64_t)n_events * (D.P.n_bins + 1) * sizeof(unsigned long long);
   CEL_CUDA(c, cudaMallocAsync(&c->d_tally, tally_bytes > 0 ? tally_bytes : 8, s));
-  D.tile_vac = (uint32_t*)((char*)c->scratch + o_vac);
-  D.tile_hist = (uint32_t*)((char*)c->scratch + o_hist);
-  D.tile_phist = (uint32_t*)((char*)c->scratch + o_phist);
-  D.tile_sec = (uint32_t*)((char*)c->scratch + o_sec);
-  D.part_cnt = (uint32_t*)((char*)c->scratch + o_part);
-  D.tile_filled = (uint32_t*)((char*)c->scratch + o_filled);
-  D.group_hist = (uint32_t*)((char*)c->scratch + o_group);
-  D.group_phist = (uint32_t*)((char*)c->scratch + o_group + group_bytes);
+  char* sb = (char*)c->scratch;
+  D.tile_vac = (uint32_t*)(sb + o_vac); D.tile_sec = (uint32_t*)(sb + o_sec);
+  D.tile_hist = (uint32_t*)(sb + o_hist); D.tile_phist = (uint32_t*)(sb + o_phist);
+  D.group_rows = (uint32_t*)(sb + o_rows); D.group_mask = (uint32_t*)(sb + o_gmask); D.part_cnt = (uint32_t*)(sb + o_part);
   D.tally = (unsigned long long*)c->d_tally;
   D.n_events = n_events;
   if (c->d_trace) { CEL_CUDA(c, cudaFreeAsync(c->d_trace, s)); c->d_trace = nullptr; }
@@ -819,8 +825,12 @@ extern "C" int cel_debug_read_indices(cel_ctx* c, uint32_t* idx, uint32_t* offse
   std::memcpy(offsets, c->last.offsets, 9 * sizeof(uint32_t));
   if (c->D.sort_mode == CEL_SORT_NONE || c->D.sort_mode == CEL_SORT_PARTITION) {
     for (uint64_t i = 0; i < c->n_slots; ++i) idx[i] = (uint32_t)i;
-  } else {
-    CEL_CUDA(c, cudaMemcpyAsync(idx, c->D.indices, c->n_slots * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+  } else {   // the index array is kept in regions of N entries per sort key: compact them into the permutation of S2
+    const int n_keys = c->D.sort_mode == CEL_SORT_BY_ACTION ? 8 : 4;
+    for (int k = 0; k < n_keys; ++k) {
+      const uint32_t n = offsets[k + 1] - offsets[k];
+      if (n) CEL_CUDA(c, cudaMemcpyAsync(idx + offsets[k], c->D.indices + (uint64_t)k * c->n_slots, (uint64_t)n * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    }
     CEL_CUDA(c, cudaStreamSynchronize(c->stream));
   }
   return CEL_OK;

@@ -92,14 +92,17 @@ struct Params {
 
 // ---------------------------------------------------------------- per-run device state
 // Bookkeeping tiles: a tile is `tile_slots` = 2^tile_shift consecutive slots, processed by one block in sub-tiles of
-// kSub slots; the tile size grows with N so that there are never more than kMaxTiles tiles, and every block can
-// form its own exclusive prefix over the per-tile counters with one block reduction (no look-back, no extra pass).
+// kSub slots; tiles are grouped by kGroupTiles for the two-level counters (cel_kernels.cuh). The tile size grows with N
+// so that there are never more than kMaxGroups groups.
 constexpr int kTileThreads = 256;
 constexpr int kKeysPerThread = 4;
 constexpr int kSub = kTileThreads * kKeysPerThread;  // 1024 slots per sub-tile
-constexpr int kMaxTiles = 4096;
+constexpr int kGroupTiles = 32;
+constexpr int kMaxGroups = 128;
+constexpr int kMaxTiles = kMaxGroups * kGroupTiles;  // 4096
+constexpr int kRowWords = 16;                        // one group row: 8 action counts, 4 particle-key counts, arrivals, tile mask, pad
 
-// index ranges of the action kernels in the sorted index array (S2)
+// index ranges of the action kernels in the index array (S2); each kernel walks up to two ranges
 enum KernelRange : int { R_PE = 0, R_PAIR, R_ANNIH, R_PHOTON, R_CHARGED, R_COUNT };
 
 struct Control {
@@ -110,10 +113,9 @@ struct Control {
   uint32_t alive;                   // A_k (after P1)
   uint32_t finished;                // A_k == 0 and I == 0
   int32_t error;
-  uint32_t offsets[9];              // offsets of the sorted index array, per sort key
+  uint32_t offsets[9];              // compact offsets of the sorted index array, per sort key (S2; debug surface)
   uint32_t counts[8];               // action counts of this iteration (after P1)
-  uint32_t rb[8], re[8];            // index range of each action kernel for this iteration (KernelRange)
-  uint32_t ticket_fill, ticket_push;
+  uint32_t rb[R_COUNT][2], re[R_COUNT][2];   // index ranges of each action kernel for this iteration (KernelRange)
   uint32_t n_logged;
   uint32_t vac_total;               // V before the fill of this iteration
   unsigned long long n_init_fill;   // I after the fill of this iteration (= n_init until k_push adds S)
@@ -126,6 +128,7 @@ struct DeviceState {
   Params P;
   uint32_t N;             // n_slots
   uint32_t n_tiles;
+  uint32_t n_groups;      // ceil(n_tiles / kGroupTiles)
   uint32_t tile_shift;    // log2(tile_slots)
   uint32_t subs_per_tile; // tile_slots / kSub
   int sort_mode;          // 0 none, 1 by action, 2 by particle, 3 partition (CEL_SORT_BY_ACTION_REUSE is 1 here, with reuse = 1)
@@ -137,20 +140,21 @@ struct DeviceState {
   RecA* stA; RecB* stB;
   uint8_t* akey;          // [n_tiles * tile_slots] action | ptype << 4; padding bytes are 0xff
   uint8_t* nsec;          // [n_tiles * tile_slots] secondaries staged by the slot in this iteration (0..2)
-  uint32_t* indices;      // [N] (sorted modes)
+  uint32_t* indices;      // sorted modes: [n_keys][N], region k = the slots of sort key k in ascending order (state_indices,
+                          // PAPER.md:41, kept per key so that a tile's write position depends only on the tiles before it);
+                          // sort mode 3: [N] the partitioned pop positions (plist, S9-P)
   RecA* secA; RecB* secB; // [2N] staged secondaries
   RecA* initA; RecB* initB; // [init_capacity]
   unsigned long long* tally; // [n_events][n_bins+1]
   uint32_t* counts_log;   // [log_capacity][8]
   Control* ctl;
   // stream-ordered scratch (cudaMallocAsync, per transport call)
-  uint32_t* tile_vac;     // [n_tiles] vacant slots per tile: += by the action kernels, -= by the fill
+  uint32_t* tile_vac;     // [2][n_tiles] vacant slots per tile, double-buffered by iteration parity (cel_kernels.cuh)
   uint32_t* tile_sec;     // [n_tiles] secondaries staged per tile in this iteration: += by the action kernels
-  uint32_t* tile_hist;    // [n_tiles][8] per-tile action histogram (-> exclusive base per key after k_init_fill, sort by action)
-  uint32_t* tile_phist;   // [n_tiles][8] per-tile particle histogram, 4 used (sort by particle)
-  uint32_t* group_hist;   // [2][kMaxGroups][8] action counts per group of 32 tiles, double-buffered by iteration parity
-  uint32_t* group_phist;  // [2][kMaxGroups][8] the same for the particle sort keys
-  uint32_t* tile_filled;  // [n_tiles] vacancies of the tile that k_init_fill filled in this iteration (k_scatter takes them off tile_vac)
+  uint32_t* tile_hist;    // [n_tiles][8] per-tile action histogram
+  uint32_t* tile_phist;   // [n_tiles][4] per-tile particle-key histogram (sort by particle)
+  uint32_t* group_rows;   // [2][kMaxGroups][kRowWords] group histograms + arrival counters, double-buffered by iteration parity
+  uint32_t* group_mask;   // [2][kMaxGroups / 32] bit g = every tile of group g has published its rows of this iteration
   uint32_t* part_cnt;     // [n_tiles] sort mode 3: charged pops per tile-sized chunk of the popped segment
   // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
   // in / last warp out of every kernel of every iteration; nullptr = off
@@ -160,7 +164,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_INIT_FILL = 0, K_SCATTER, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
+enum KernelId : int { K_FILL_SORT = 0, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
@@ -205,7 +209,7 @@ struct TraceScope<KID, true> {
 };
 
 // ---------------------------------------------------------------- programmatic dependent launch (sm_90+)
-// The kernels of the main-stream chain (fill -> scatter -> charged -> push -> next fill) are launched with the
+// The kernels of the main-stream chain (fill_sort -> charged -> push -> next fill_sort) are launched with the
 // programmatic-stream-serialization attribute: a kernel lets its successor's blocks be scheduled early
 // (launch_dependents) and waits itself, before touching any memory, until its predecessors have completed and
 // flushed (wait). Without the attribute both instructions are no-ops.

@@ -1,18 +1,26 @@
 // cel_kernels.cuh — the bookkeeping kernels of one step iteration (docs/PHYSICS_SPEC.md S1):
-//   P1 init + P2 histogram: k_init_fill   (scan-based vacancy filling, S9; per-tile sort-key histogram, S2)
-//   P2 reindex:             k_scatter     (closes the fill: vacancy counters, action counts, offsets, control block;
-//                                          then the stable counting sort of slot indices, S2)
+//   P1 init + P2 reindex:   k_fill_sort   (scan-based vacancy filling, S9; stable counting sort of slot indices, S2;
+//                                          the iteration's counts, ranges and counters, S11) — ONE pass, one launch
 //   P5 push:                k_push        (scan-ordered secondary push, S9)
 //   S9-P (sort mode 3):     k_part_count, k_part_scatter (charged / neutral partition of the popped initializers)
 // (P3/P4, the action kernels and the scoring, are in cel_physics.cuh.)
-// No kernel has a "last block" phase: what one block would have to do after all the others (scans over tiles, the
-// control block) is either done redundantly by every block from small two-level counters, or left to the blocks of
-// the next kernel.
-// The action kernels keep two per-tile counters up to date with integer atomics — vacancies created and secondaries
-// staged — so neither scan needs a counting pass: a block reduces the counters of the tiles before it to get its
-// exclusive prefix, skips its tile when there is nothing to fill / push, and otherwise scans the tile's dense key
-// bytes (1 B per slot) in sub-tiles of 1024 slots. The record copies (64 B per initializer) are spread over the
-// whole block through a compacted work list in shared memory, 32 B per thread and step.
+//
+// One 256-thread block per tile of 2^tile_shift consecutive slots. What makes a single pass possible:
+//  * the action kernels keep per-tile counters of vacancies created and secondaries staged (integer atomics), so a
+//    block gets its exclusive prefix from one strided read of <= 4096 counters — no counting pass, no look-back chain;
+//  * the index array is kept in REGIONS of N entries, one per sort key: region k holds the slots of key k in ascending
+//    order from k*N, so where a tile writes depends only on the tiles BEFORE it (their per-key counts), never on
+//    totals. A block publishes its tile's histogram (own row + atomics on its group's row), then waits for the tiles
+//    before it — whole lower groups through an arrival counter in the group row, lower tiles of its own group through
+//    a per-tile iteration stamp — and scatters from the key bytes it still holds in shared memory. Dependencies point
+//    only to lower block indices, which the hardware dispatches first, so the wait cannot deadlock even when the
+//    grid is only partly resident (several contexts sharing the GPU); a bounded spin turns the impossible case into
+//    the sticky error CEL_ERR_INTERNAL instead of a hang.
+//  * the block of the LAST tile, which by then has seen every other tile's counts, writes the iteration's totals,
+//    ranges and counters to the control block (fields no block of this kernel reads).
+// The vacancy counters are double-buffered by the parity of the iteration: fill(k) reads buffer k&1 (complete once the
+// action kernels of k-1 are), writes what is left of its tile into buffer (k&1)^1, which the action kernels of k then
+// add to. So the prefix can be formed BEFORE the programmatic-dependency wait and overlaps the push of the previous iteration.
 #pragma once
 #include "cel_device.cuh"
 
@@ -66,77 +74,6 @@ __device__ __forceinline__ unsigned long long block_excl_scan64(unsigned long lo
   total = smem[8];
   return smem[warp] + incl - v;
 }
-// in-place exclusive scan of a[0..n) (stride in words) by one block; returns the total to every thread
-__device__ __forceinline__ uint32_t block_scan_array(uint32_t* a, uint32_t n, uint32_t stride, uint32_t* smem) {
-  __shared__ uint32_t carry_s;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  for (uint32_t base = 0; base < n; base += kTileThreads) {
-    uint32_t i = base + threadIdx.x;
-    uint32_t v = (i < n) ? a[(size_t)i * stride] : 0;
-    uint32_t total;
-    uint32_t ex = block_excl_scan(v, smem, total);
-    uint32_t carry = carry_s;
-    if (i < n) a[(size_t)i * stride] = carry + ex;
-    __syncthreads();
-    if (threadIdx.x == 0) carry_s = carry + total;
-    __syncthreads();
-  }
-  return carry_s;
-}
-// sum of a[0..tile) and of a[0..n) by one block (n <= kMaxTiles): the block's exclusive prefix and the grand total
-__device__ __forceinline__ void block_prefix_total(const uint32_t* a, uint32_t n, uint32_t tile, uint32_t* smem /* 18 words */,
-                                                   uint32_t& prefix, uint32_t& total) {
-  uint32_t p = 0, t = 0;
-  for (uint32_t i = threadIdx.x; i < n; i += kTileThreads) {
-    const uint32_t v = a[i];
-    t += v;
-    if (i < tile) p += v;
-  }
-  p = __reduce_add_sync(0xffffffffu, p);
-  t = __reduce_add_sync(0xffffffffu, t);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  __syncthreads();
-  if (lane == 0) { smem[warp] = p; smem[9 + warp] = t; }
-  __syncthreads();
-  p = 0; t = 0;
-#pragma unroll
-  for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
-  prefix = p; total = t;
-}
-// The same with the counters already in registers: load_counters issues every load of the kernel's prologue back to
-// back (control block, counters) BEFORE the first use, so the prologue costs one L2 round trip instead of one per
-// dependent step (in-order issue stalls at the first use). Also returns a[tile].
-// (CPT counters per thread: 8 up to 2048 tiles, 16 above — two instantiations of the kernels that use it, so that the
-// common sizes keep their register count)
-template <int CPT>
-__device__ __forceinline__ void load_counters(const uint32_t* a, uint32_t n, uint32_t (&v)[CPT]) {
-#pragma unroll
-  for (int i = 0; i < CPT; ++i) { const uint32_t idx = threadIdx.x + i * kTileThreads; v[i] = idx < n ? a[idx] : 0u; }
-}
-template <int CPT>
-__device__ __forceinline__ void block_prefix_total_regs(const uint32_t (&v)[CPT], uint32_t tile, uint32_t* smem /* 19 words */,
-                                                        uint32_t& prefix, uint32_t& total, uint32_t& own) {
-  uint32_t p = 0, t = 0;
-#pragma unroll
-  for (int i = 0; i < CPT; ++i) {
-    const uint32_t idx = threadIdx.x + i * kTileThreads;
-    t += v[i];
-    if (idx < tile) p += v[i];
-  }
-  p = __reduce_add_sync(0xffffffffu, p);
-  t = __reduce_add_sync(0xffffffffu, t);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  __syncthreads();
-  if (lane == 0) { smem[warp] = p; smem[9 + warp] = t; }
-#pragma unroll
-  for (int i = 0; i < CPT; ++i) if (threadIdx.x + i * kTileThreads == tile) smem[18] = v[i];
-  __syncthreads();
-  p = 0; t = 0;
-#pragma unroll
-  for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
-  prefix = p; total = t; own = smem[18];
-}
 __device__ __forceinline__ int sort_key_of(int sort_mode, uint32_t key) {
   const int a = key & 0xf;
   if (sort_mode == 1) return a;
@@ -149,25 +86,74 @@ __device__ __forceinline__ uint32_t count_vacant4(uint32_t w) {
   return __popc(z);
 }
 
+// loads that must see what other SMs published through L2 (atomics / stores + fence): never from L1
+__device__ __forceinline__ uint32_t load_acquire(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void store_release(uint32_t* p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
 // ---------------------------------------------------------------- shared memory of a bookkeeping block
+constexpr int kResidentSubs = 4;   // sub-tiles whose key bytes stay in shared memory between the fill and the scatter
 struct BookSmem {
   uint32_t scan[20];
   unsigned long long scan64[9];
   uint32_t hist[8], act[8], base[8];
-  uint32_t skey[kTileThreads];   // the sub-tile's key bytes
-  uint32_t list[2 * kSub];       // compacted work list of the cooperative copies
+  uint32_t part[3 * 9];            // per-warp partial sums of the prefix reductions
+  uint32_t before[12];             // per-key counts of the tiles before this one: 0-7 action keys, 8-11 particle keys
+  uint32_t skey[kResidentSubs * kTileThreads];   // key bytes of the tile's sub-tiles
+  uint32_t list[2 * kSub];         // compacted work list of the cooperative copies
 };
 
 __device__ __forceinline__ uint32_t real_slots_in_tile(const DeviceState& D, uint32_t tile) {
   const unsigned long long lo = (unsigned long long)tile << D.tile_shift, hi = lo + (1ull << D.tile_shift);
   return lo >= D.N ? 0u : (uint32_t)((hi < D.N ? hi : (unsigned long long)D.N) - lo);
 }
+__device__ __forceinline__ uint32_t tiles_in_group(const DeviceState& D, uint32_t g) {
+  const uint32_t lo = g * kGroupTiles;
+  return lo >= D.n_tiles ? 0u : min((uint32_t)kGroupTiles, D.n_tiles - lo);
+}
+
+// Exclusive prefix of a per-tile counter by one block: the sum over the tiles before `tile`, the grand total and the tile's
+// own counter. Threads stride over all the counters (n_tiles <= 4096: at most 16 loads per thread, issued back to back before
+// the first use: one L2 round trip). Uses sm.part; ends with a barrier.
+__device__ __forceinline__ void tile_prefix(const DeviceState& D, BookSmem& sm, const uint32_t* tile_cnt, uint32_t tile,
+                                            uint32_t& prefix, uint32_t& total, uint32_t& own) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint32_t before = 0, all = 0, mine = 0;
+  for (uint32_t i0 = 0; i0 < D.n_tiles; i0 += 4 * kTileThreads) {
+    uint32_t v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const uint32_t i = i0 + u * kTileThreads + threadIdx.x; v[u] = i < D.n_tiles ? __ldcg(tile_cnt + i) : 0u; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + u * kTileThreads + threadIdx.x;
+      all += v[u];
+      if (i < tile) before += v[u];
+      if (i == tile) mine = v[u];
+    }
+  }
+  before = __reduce_add_sync(0xffffffffu, before);
+  all = __reduce_add_sync(0xffffffffu, all);
+  mine = __reduce_add_sync(0xffffffffu, mine);
+  __syncthreads();
+  if (lane == 0) { sm.part[warp] = before; sm.part[9 + warp] = all; sm.part[18 + warp] = mine; }
+  __syncthreads();
+  uint32_t p = 0, t = 0, o = 0;
+#pragma unroll
+  for (int w = 0; w < kTileThreads / 32; ++w) { p += sm.part[w]; t += sm.part[9 + w]; o += sm.part[18 + w]; }
+  prefix = p; total = t; own = o;
+}
 
 // ================================================================ P1: vacancy scan + fill (S9), P2 histogram (S2)
 // Rank-r vacant slot (ascending slot order) takes init[I-1-r] when r < I (LIFO). The rank of a tile's first vacancy
-// (`prefix`) is the sum of tile_vac over the tiles before it — scan-based, no atomics in the assignment, so the slot
+// (`prefix`) comes from the two-level vacancy counters — scan-based, no atomics in the assignment, so the slot
 // assignment is deterministic. Adds the tile's action histogram to sm.act and (sort by particle) its
-// sort-key histogram to sm.hist; the caller zeroes both and synchronises before, and synchronises after.
+// sort-key histogram to sm.hist; the caller zeroes both and synchronises before, and synchronises after. Leaves the
+// (updated) key bytes of the first kResidentSubs sub-tiles in sm.skey.
 // Which vacancies are filled: ranks [0, low_n) and [high_start, V). Plain rule (S9): low_n = n_take, high_start = V
 // (none at the high end), rank r takes pop position r. Partition rule (S9-P, sort mode 3): low_n = C charged,
 // high_start = V - G neutral; rank r < C takes the pop position plist[r], rank r >= V - G takes plist[n_take-1-(V-1-r)]
@@ -184,25 +170,28 @@ __device__ __forceinline__ uint32_t filled_by_plan(uint32_t v, uint32_t prefix, 
   const uint32_t hs = max(prefix, pl.high_start);
   return lo + (end > hs ? end - hs : 0u);
 }
-__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, const FillPlan pl,
+// returns true if the tile's key bytes were read (false: the tile is entirely vacant and gets no fill)
+__device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, const FillPlan pl,
                                           uint32_t prefix, uint32_t tile_vacant) {
   uint32_t rank0 = prefix;                                   // rank of the first vacancy of the current sub-tile
   const uint32_t rank_end = prefix + tile_vacant;            // one past the rank of the tile's last vacancy
   const uint32_t real = real_slots_in_tile(D, tile);
-  if (tile_vacant == real && filled_by_plan(tile_vacant, prefix, pl) == 0) {   // all vacant, nothing to fill: no key byte needs reading
-    if (threadIdx.x == 0) { atomicAdd(&sm.act[A_VACANT], real); if (D.sort_mode == 2) atomicAdd(&sm.hist[3], real); }
-    return;
+  // all vacant, nothing to fill: no key byte needs reading (unless the debug surface wants the vacant indices written too)
+  if (!D.write_vacant && tile_vacant == real && filled_by_plan(tile_vacant, prefix, pl) == 0) {
+    if (threadIdx.x == 0) { sm.act[A_VACANT] = real; if (D.sort_mode == 2) sm.hist[3] = real; }
+    return false;
   }
-  uint8_t* skey_b = reinterpret_cast<uint8_t*>(sm.skey);
   for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
     const uint32_t sub_base = (tile << D.tile_shift) + sub * kSub;
     const uint32_t base = sub_base + threadIdx.x * kKeysPerThread;
     uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
+    uint32_t* skey = sm.skey + (sub < (uint32_t)kResidentSubs ? sub : 0u) * kTileThreads;   // (beyond kResidentSubs: scratch only)
+    uint8_t* skey_b = reinterpret_cast<uint8_t*>(skey);
     if (rank0 < rank_end && filled_by_plan(rank_end - rank0, rank0, pl) != 0) {   // block-uniform: this sub-tile may have vacancies to fill
       const uint32_t c = count_vacant4(kv);
       uint32_t total;
       uint32_t r = block_excl_scan(c, sm.scan, total);
-      sm.skey[threadIdx.x] = kv;
+      skey[threadIdx.x] = kv;
       if (c) {
 #pragma unroll
         for (int i = 0; i < kKeysPerThread; ++i)
@@ -213,7 +202,9 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
       const uint32_t n_lo = pl.low_n > rank0 ? min(total, pl.low_n - rank0) : 0u;
       const uint32_t hi_begin = pl.high_start > rank0 ? min(total, pl.high_start - rank0) : 0u;
       const uint32_t nf = n_lo + (total - hi_begin);
-      // cooperative copy: work item w = (record, half); half 0 = RecA, half 1 = RecB (+ the key byte)
+      // cooperative copy: work item w = (record, half); half 0 = RecA, half 1 = RecB (+ the key byte).
+      // (Tried: two passes in flight per thread through cp.async landing slots in shared memory — 16 KB more shared
+      // memory per block cost more in lost overlap with the neighbouring kernels than the pipelining gained: +7 %.)
       for (uint32_t w = threadIdx.x; w < 2 * nf; w += kTileThreads) {
         const uint32_t m = w >> 1;
         const uint32_t item = m < n_lo ? m : hi_begin + (m - n_lo);
@@ -233,8 +224,10 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
         }
       }
       __syncthreads();
-      kv = sm.skey[threadIdx.x];
+      kv = skey[threadIdx.x];
       rank0 += total;
+    } else if (sub < (uint32_t)kResidentSubs) {
+      skey[threadIdx.x] = kv;
     }
     // histograms of this thread's 4 keys, 8 x 8-bit packed (padding bytes 0xff are skipped)
     uint32_t a_lo = 0, a_hi = 0, s_lo = 0;
@@ -260,71 +253,27 @@ __device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, ui
       }
     }
   }
+  return true;
 }
-__device__ __forceinline__ void fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t n_take,
-                                          uint32_t prefix, uint32_t tile_vacant) {
-  fill_tile(D, sm, tile, I, plain_plan(n_take), prefix, tile_vacant);
-}
-// Two-level histograms. Besides its own row tile_hist[tile][8], every fill block adds its counts into the row of its
-// GROUP of kGroupTiles tiles (integer atomics on 8 x n_groups addresses, double-buffered by the parity of the iteration:
-// the blocks of iteration k also zero the rows that iteration k+1 will add into). Column totals are then the sum of
-// <= 128 group rows, and the base of a tile in the counting sort is (groups before its group) + (tiles of its group
-// before it): 2 KB read by each scatter block, 2 KB by the one block that updates the control block — instead of one
-// block scanning all 32 KB of rows in place, which was 4.4 of the 12 us of an almost empty k_init_fill (one SM pulls
-// ~64 B per clock from L2; profiles/).
-constexpr int kGroupTiles = 32;
-constexpr int kMaxGroups = kMaxTiles / kGroupTiles;   // 128
-__device__ __forceinline__ uint32_t* group_rows(uint32_t* base, uint32_t parity) { return base + (size_t)parity * kMaxGroups * 8; }
-// after fill_tile + __syncthreads: publish the tile's action histogram and (sort by particle) its sort-key histogram.
-// The iteration's action counts are the column sums of tile_hist (no same-address atomics from a thousand blocks).
-__device__ __forceinline__ void publish_tile_hist(const DeviceState& D, BookSmem& sm, uint32_t tile) {
-  if (threadIdx.x < 8) {
-    D.tile_hist[tile * 8 + threadIdx.x] = sm.act[threadIdx.x];
-    if (D.sort_mode == 2) D.tile_phist[tile * 8 + threadIdx.x] = threadIdx.x < 4 ? sm.hist[threadIdx.x] : 0u;
-  }
-}
-// the kernel-per-action form: the group rows of the two-level histograms (see group_rows)
-__device__ __forceinline__ void publish_group_hist(const DeviceState& D, BookSmem& sm, uint32_t tile, uint32_t parity) {
-  if (threadIdx.x < 8) {
-    const uint32_t g = tile / kGroupTiles;
-    const uint32_t a = sm.act[threadIdx.x];
-    if (a) atomicAdd(group_rows(D.group_hist, parity) + g * 8 + threadIdx.x, a);
-    if (D.sort_mode == 2 && threadIdx.x < 4) { const uint32_t h = sm.hist[threadIdx.x]; if (h) atomicAdd(group_rows(D.group_phist, parity) + g * 8 + threadIdx.x, h); }
-    if (tile < (uint32_t)kMaxGroups) {   // the rows the next iteration adds into (last read by the previous iteration's scatter)
-      group_rows(D.group_hist, parity ^ 1u)[tile * 8 + threadIdx.x] = 0u;
-      if (D.sort_mode == 2) group_rows(D.group_phist, parity ^ 1u)[tile * 8 + threadIdx.x] = 0u;
-    }
-  }
-}
-// the rows the scatter takes its per-tile bases from: the action histogram (sort by action) or the particle histogram
-__device__ __forceinline__ uint32_t* sort_rows(const DeviceState& D) { return D.sort_mode == 2 ? D.tile_phist : D.tile_hist; }
 
-// sum over the rows r < n_rows (n_rows <= 32) of rows[r][0..8) by one warp; every lane gets the 8 column sums
-__device__ __forceinline__ void warp_sum_rows(const uint32_t* rows, uint32_t n_rows, uint32_t* out8) {
-  const uint32_t lane = threadIdx.x & 31;
-  uint4 a = make_uint4(0, 0, 0, 0), b = make_uint4(0, 0, 0, 0);
-  if (lane < n_rows) { a = *reinterpret_cast<const uint4*>(rows + lane * 8); b = *reinterpret_cast<const uint4*>(rows + lane * 8 + 4); }
-  out8[0] = __reduce_add_sync(0xffffffffu, a.x); out8[1] = __reduce_add_sync(0xffffffffu, a.y);
-  out8[2] = __reduce_add_sync(0xffffffffu, a.z); out8[3] = __reduce_add_sync(0xffffffffu, a.w);
-  out8[4] = __reduce_add_sync(0xffffffffu, b.x); out8[5] = __reduce_add_sync(0xffffffffu, b.y);
-  out8[6] = __reduce_add_sync(0xffffffffu, b.z); out8[7] = __reduce_add_sync(0xffffffffu, b.w);
+// Group rows of the two-level histograms: [2 (iteration parity)][kMaxGroups][kRowWords]; words 0-7 action counts of the
+// group's tiles, 8-11 particle-key counts (sort by particle), 12 the number of tiles of the group that have published.
+// The blocks of iteration k add into the rows of parity k&1 and zero the rows iteration k+1 will add into.
+__device__ __forceinline__ uint32_t* group_row(const DeviceState& D, uint32_t parity, uint32_t g) {
+  return D.group_rows + ((size_t)parity * kMaxGroups + g) * kRowWords;
 }
-// vacancies of a tile that the fill of this iteration takes: min(v, max(0, n_take - (vacancies before the tile)))
-__device__ __forceinline__ uint32_t filled_in_tile(uint32_t v, uint32_t prefix, uint32_t n_take) {
-  return min(v, n_take > prefix ? n_take - prefix : 0u);
-}
+constexpr uint32_t kSpinLimit = 1u << 24;   // polls before a wait gives up (~ a second): CEL_ERR_INTERNAL instead of a hang
 
 // ================================================================ P2: stable scatter of slot indices (S2)
-// indices[offset[key] + (tiles before)[key] + (rank inside the tile)] = slot; ascending slot order inside a key.
-// The caller sets sm.base[key] = offset[key] + (tiles before)[key] and synchronises. Vacant slots are never launched:
-// their indices are written only when the complete permutation is asked for (debug surface), and a tile that is
-// entirely vacant is then skipped without reading its key bytes.
-__device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, uint32_t tile_vacant_now) {
+// indices[region(key) + (tiles before)[key] + (rank inside the tile)] = slot; ascending slot order inside a key.
+// The caller sets sm.base[key] and synchronises. Vacant slots are never launched: their indices are written only when
+// the complete permutation is asked for (debug surface). Key bytes come from shared memory (left there by fill_tile) for
+// the first kResidentSubs sub-tiles.
+__device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm, uint32_t tile) {
   const int vacant_key = D.sort_mode == 1 ? (int)A_VACANT : 3;
-  if (!D.write_vacant && tile_vacant_now == real_slots_in_tile(D, tile)) return;
   for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
     const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
-    const uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
+    const uint32_t kv = sub < (uint32_t)kResidentSubs ? sm.skey[sub * kTileThreads + threadIdx.x] : *reinterpret_cast<const uint32_t*>(D.akey + base);
     // per-thread key counts, 4 x 16-bit packed in two words (keys 0-3, 4-7); a sub-tile has 1024 slots < 2^16
     unsigned long long lo = 0, hi = 0;
 #pragma unroll
@@ -347,7 +296,7 @@ __device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm,
         uint32_t r;
         if (s < 4) { r = (uint32_t)((plo >> (16 * s)) & 0xffff); plo += 1ull << (16 * s); }
         else { r = (uint32_t)((phi >> (16 * (s - 4))) & 0xffff); phi += 1ull << (16 * (s - 4)); }
-        if (s != vacant_key || D.write_vacant) D.indices[sm.base[s] + r] = base + i;
+        if (s != vacant_key || D.write_vacant) D.indices[(size_t)s * D.N + sm.base[s] + r] = base + i;
       }
     }
     if (sub + 1 < D.subs_per_tile) {   // advance the per-key bases by this sub-tile's totals
@@ -362,7 +311,7 @@ __device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm,
 // ================================================================ P5: secondary push (S9)
 // Exclusive scan of nsec[slot] in ascending SLOT order (in every sort mode), so that the initializer order — and with
 // it every later slot assignment and PRNG stream — does not depend on thread timing or on the sort mode. A tile's
-// offset `off0` is the sum of tile_sec over the tiles before it; a tile that staged nothing is not read at all.
+// offset `off0` comes from the two-level counters of staged secondaries; a tile that staged nothing is not read at all.
 __device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t off0,
                                           uint32_t tile_total, bool overflow) {
   const uint32_t off_end = off0 + tile_total;
@@ -396,49 +345,49 @@ __device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, ui
   }
 }
 
-// S2: the index range of each action kernel from the key offsets
-__device__ __forceinline__ void set_ranges(const DeviceState& D, const uint32_t* off, uint32_t* rb, uint32_t* re) {
-  if (D.sort_mode == 1) {        // PE | PAIR | COMPTON MOVE_G | MOVE_C BREMS | ANNIH | VACANT
-    rb[R_PE] = off[0]; re[R_PE] = off[1];
-    rb[R_PAIR] = off[1]; re[R_PAIR] = off[2];
-    rb[R_PHOTON] = off[2]; re[R_PHOTON] = off[4];
-    rb[R_CHARGED] = off[4]; re[R_CHARGED] = off[6];
-    rb[R_ANNIH] = off[6]; re[R_ANNIH] = off[7];
-  } else if (D.sort_mode == 2) { // gamma | e- | e+ | vacant
-    rb[R_PE] = rb[R_PAIR] = rb[R_PHOTON] = off[0];
-    re[R_PE] = re[R_PAIR] = re[R_PHOTON] = off[1];
-    rb[R_CHARGED] = off[1]; re[R_CHARGED] = off[3];
-    rb[R_ANNIH] = off[2]; re[R_ANNIH] = off[3];
+// S2: the index ranges of each action kernel. Sorted modes: region k of the index array is [k N, k N + total[k]).
+__device__ __forceinline__ void set_ranges(const DeviceState& D, const uint32_t* key_total, Control* ctl) {
+  for (int r = 0; r < R_COUNT; ++r) for (int j = 0; j < 2; ++j) { ctl->rb[r][j] = 0; ctl->re[r][j] = 0; }
+  const uint32_t N = D.N;
+  auto region = [&](int r, int j, int key) { ctl->rb[r][j] = (uint32_t)key * N; ctl->re[r][j] = (uint32_t)key * N + key_total[key]; };
+  if (D.sort_mode == 1) {        // one region per action
+    region(R_PE, 0, A_PE); region(R_PAIR, 0, A_PAIR); region(R_ANNIH, 0, A_ANNIH);
+    region(R_PHOTON, 0, A_COMPTON); region(R_PHOTON, 1, A_MOVE_G);
+    region(R_CHARGED, 0, A_BREMS); region(R_CHARGED, 1, A_MOVE_C);
+  } else if (D.sort_mode == 2) { // regions gamma | e- | e+ ; the kernels mask by action inside their particle's regions
+    region(R_PE, 0, 0); region(R_PAIR, 0, 0); region(R_PHOTON, 0, 0);
+    region(R_CHARGED, 0, 1); region(R_CHARGED, 1, 2);
+    region(R_ANNIH, 0, 2);
   } else {
-    for (int k = 0; k < R_COUNT; ++k) { rb[k] = 0; re[k] = D.N; }
+    for (int r = 0; r < R_COUNT; ++r) { ctl->rb[r][0] = 0; ctl->re[r][0] = N; }
   }
 }
-// end-of-P1 bookkeeping of the control block by one thread (S11): counts, offsets, ranges, I, alive, log
+// end-of-P1 bookkeeping of the control block by one thread (S11): counts, offsets, ranges, I, alive, log. The running
+// counters (only this thread ever writes them) were read in the kernel's prologue, so everything here is a store.
+struct ControlCarry { unsigned long long track_steps, iterations; uint32_t n_logged; };
 __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, const uint32_t* act_total, const uint32_t* key_total,
-                                                          int n_keys, unsigned long long I, uint32_t V, uint32_t n_take) {
+                                                          int n_keys, unsigned long long Iafter, uint32_t V, uint32_t iter, const ControlCarry cc) {
   Control* ctl = D.ctl;
   uint32_t cnt[8];
   for (int a = 0; a < 8; ++a) { cnt[a] = act_total[a]; ctl->counts[a] = cnt[a]; }
   const uint32_t N = D.N;
-  uint32_t off[9];
+  uint32_t off[9];   // the compact offsets of S2 (what the debug surface reports; the kernels use the regions)
   off[0] = 0;
   for (int k = 0; k < 8; ++k) off[k + 1] = (k < n_keys) ? off[k] + key_total[k] : off[k];
   if (n_keys == 0) for (int k = 1; k <= 8; ++k) off[k] = N;
   for (int k = 0; k <= 8; ++k) ctl->offsets[k] = off[k];
-  set_ranges(D, off, ctl->rb, ctl->re);
+  set_ranges(D, key_total, ctl);
   const uint32_t alive = N - cnt[A_VACANT];
-  const unsigned long long Iafter = I - n_take;   // I -= min(V, I)
   ctl->vac_total = V;
-  ctl->n_init = Iafter;
   ctl->n_init_fill = Iafter;   // what k_push reads (it writes n_init itself)
-  ctl->iter_cur = ctl->iter;
+  ctl->iter_cur = iter;
   ctl->alive = alive;
   if (alive == 0 && Iafter == 0) {
     ctl->finished = 1;
   } else {
-    ctl->track_steps += alive;
-    ctl->iterations += 1;
-    const uint32_t k = ctl->n_logged;
+    ctl->track_steps = cc.track_steps + alive;
+    ctl->iterations = cc.iterations + 1;
+    const uint32_t k = cc.n_logged;
     if (k < D.log_capacity) {
       for (int a = 0; a < 8; ++a) D.counts_log[(size_t)k * 8 + a] = cnt[a];
       ctl->n_logged = k + 1;
@@ -446,136 +395,145 @@ __device__ __forceinline__ void update_control_after_fill(const DeviceState& D, 
   }
 }
 
-// ================================================================ the bookkeeping kernels (one block per tile)
-// k_init_fill: P1 + the per-tile and per-group histograms.
-template <bool TRACE, int CPT>
-__global__ void __launch_bounds__(kTileThreads) k_init_fill(DeviceState D) {
+// ================================================================ k_fill_sort: P1 + P2 + S11 in one pass (one block per tile)
+template <bool TRACE>
+__global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   __shared__ BookSmem sm;
   Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
-  // Before the programmatic-dependency wait: what does NOT depend on the kernel just before this one in the stream
-  // (k_push of the previous iteration, or the partition passes, which only touch the stack, its height, `iter` and
-  // plist): the vacancy counters and `finished` were last written by the action kernels / the previous k_init_fill,
-  // which had completed before that kernel let this one start. The vacancy prefix so overlaps the push.
+  const uint32_t g = tile / kGroupTiles, tg0 = g * kGroupTiles;
+  // ---- before the programmatic-dependency wait: what does NOT depend on the kernel just before this one in the stream
+  // (k_push of the previous iteration, or the partition passes, which only touch the stack, its height, `iter`, plist and
+  // the group counters of the OTHER parity): `finished`, `iter_cur` and the vacancy counters of parity k&1 were last
+  // written by the action kernels / the previous k_fill_sort, which had completed before that kernel let this one start.
   const uint32_t finished = ctl->finished;
-  uint32_t cnt[CPT];
-  load_counters<CPT>(D.tile_vac, D.n_tiles, cnt);
+  const uint32_t k = ctl->iter_cur + 1u;          // iter_cur = 0xffffffff after the reset
+  const uint32_t p = k & 1u;
+  ControlCarry cc; cc.track_steps = ctl->track_steps; cc.iterations = ctl->iterations; cc.n_logged = ctl->n_logged;   // (used by the last tile's block)
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
+  if (threadIdx.x < 12) sm.before[threadIdx.x] = 0;
   uint32_t prefix, V, tile_vacant;
-  block_prefix_total_regs<CPT>(cnt, tile, sm.scan, prefix, V, tile_vacant);   // (its barriers also publish sm.hist / sm.act)
+  tile_prefix(D, sm, D.tile_vac + (size_t)p * D.n_tiles, tile, prefix, V, tile_vacant);
   pdl_prologue();
-  const uint32_t iter = ctl->iter, n_charged = ctl->part_charged;
+  const uint32_t n_charged = ctl->part_charged;
   const unsigned long long I = ctl->n_init;
   if (finished) return;
-  const TraceScope<K_INIT_FILL, TRACE> trace(D, iter);
+  const TraceScope<K_FILL_SORT, TRACE> trace(D, k);
   if (threadIdx.x == 8) D.tile_sec[tile] = 0;   // consumed by the push of the previous iteration
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
-  fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
+  const bool keys_read = fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
   __syncthreads();
-  publish_tile_hist(D, sm, tile);
-  const uint32_t parity = iter & 1u;
-  publish_group_hist(D, sm, tile, parity);
-  // No "last block": the block leaves what it filled for k_scatter to take off tile_vac (other blocks of THIS kernel
-  // may still be reading the counters), and block 0 leaves the iteration's scalars in fields no fill block reads.
-  if (threadIdx.x == 0) {
-    D.tile_filled[tile] = filled_by_plan(tile_vacant, prefix, plan);
-    if (tile == 0) { ctl->vac_total = V; ctl->n_init_fill = I - n_take; ctl->iter_cur = iter; }
-  }
-}
-
-// k_scatter (every sort mode; "reindex + close the fill"): takes the filled vacancies off tile_vac; every block sums the <= 128 group rows into the
-// iteration's action / sort-key counts, hence the key offsets; block 0 writes them with ranges, counters and the log
-// to the control block (S11); in the sorted modes the block then scatters its tile's slot indices (P2).
-template <bool TRACE>
-__global__ void __launch_bounds__(kTileThreads) k_scatter(DeviceState D) {
-  __shared__ BookSmem sm;
-  pdl_prologue();
-  Control* ctl = D.ctl;
-  const uint32_t tile = blockIdx.x;
-  const uint32_t finished = ctl->finished, iter = ctl->iter;
-  const uint32_t tile_vacant = D.tile_vac[tile] - D.tile_filled[tile];
-  const unsigned long long Iafter = ctl->n_init_fill;
-  const uint32_t V = ctl->vac_total;
-  if (finished) return;   // (block 0 may set it below while others start: they then skip work nobody needs any more)
-  const TraceScope<K_SCATTER, TRACE> trace(D, iter);
-  if (threadIdx.x == 0) D.tile_vac[tile] = tile_vacant;
+  // ---- publish: the tile's rows, its group's rows, what is left of its vacancies; then the stamps the later tiles wait for
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
+  const bool is_last = tile == D.n_tiles - 1u;
   {
-    const uint32_t parity = iter & 1u;
-    const uint32_t n_groups = (D.n_tiles + kGroupTiles - 1) / kGroupTiles;
-    const uint32_t g = tile / kGroupTiles, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    constexpr int kGroupWarps = kMaxGroups / 32;   // 4
-    __shared__ uint32_t act_part[kGroupWarps][8], key_part[kGroupWarps][8], before[kGroupWarps + 1][8], off_s[9];
-    if (warp < (uint32_t)kGroupWarps) {   // warp w sums the group rows [32 w, 32 w + 32): all of them (totals) and those before the tile's group
-      const uint32_t row = warp * 32 + lane;
-      const uint32_t* arows = group_rows(D.group_hist, parity);
-      const uint32_t* krows = D.sort_mode == 2 ? group_rows(D.group_phist, parity) : arows;
-      uint4 a0 = make_uint4(0, 0, 0, 0), a1 = a0, k0 = a0, k1 = a0;
-      if (row < n_groups) {
-        a0 = *reinterpret_cast<const uint4*>(arows + row * 8); a1 = *reinterpret_cast<const uint4*>(arows + row * 8 + 4);
-        if (D.sort_mode == 2) { k0 = *reinterpret_cast<const uint4*>(krows + row * 8); k1 = *reinterpret_cast<const uint4*>(krows + row * 8 + 4); }
-        else { k0 = a0; k1 = a1; }
-      }
-      const uint32_t av[8] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w};
-      const uint32_t kv[8] = {k0.x, k0.y, k0.z, k0.w, k1.x, k1.y, k1.z, k1.w};
-      const bool bef = row < g;
-#pragma unroll
-      for (int k = 0; k < 8; ++k) {
-        const uint32_t ta = __reduce_add_sync(0xffffffffu, av[k]);
-        const uint32_t tk = __reduce_add_sync(0xffffffffu, kv[k]);
-        const uint32_t tb = __reduce_add_sync(0xffffffffu, bef ? kv[k] : 0u);
-        if (lane == 0) { act_part[warp][k] = ta; key_part[warp][k] = tk; before[warp][k] = tb; }
-      }
-    } else if (warp == (uint32_t)kGroupWarps) {   // the tile rows of the own group before the tile
-      uint32_t s8[8];
-      warp_sum_rows(sort_rows(D) + (size_t)g * kGroupTiles * 8, n_keys ? tile - g * kGroupTiles : 0u, s8);
-      if (lane == 0) {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) before[kGroupWarps][k] = s8[k];
-      }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      uint32_t act_total[8], key_total[8];
-      for (int k = 0; k < 8; ++k) {
-        act_total[k] = 0; key_total[k] = 0;
-        for (int w = 0; w < kGroupWarps; ++w) { act_total[k] += act_part[w][k]; key_total[k] += key_part[w][k]; }
-      }
-      uint32_t o = 0;
-      for (int k = 0; k < 8; ++k) { off_s[k] = o; if (k < n_keys) o += key_total[k]; }
-      if (tile == 0) update_control_after_fill(D, act_total, key_total, n_keys, Iafter, V, 0u);
-    }
-    __syncthreads();
+    uint32_t* row = group_row(D, p, g);
     if (threadIdx.x < 8) {
-      uint32_t b = off_s[threadIdx.x];
-      for (int w = 0; w <= kGroupWarps; ++w) b += before[w][threadIdx.x];
-      sm.base[threadIdx.x] = b;
+      const uint32_t a = sm.act[threadIdx.x];
+      D.tile_hist[(size_t)tile * 8 + threadIdx.x] = a;
+      if (a) atomicAdd(row + threadIdx.x, a);
+    } else if (threadIdx.x < 12 && D.sort_mode == 2) {
+      const uint32_t h = sm.hist[threadIdx.x - 8];
+      D.tile_phist[(size_t)tile * 4 + (threadIdx.x - 8)] = h;
+      if (h) atomicAdd(row + threadIdx.x, h);
+    } else if (threadIdx.x == 12) {
+      D.tile_vac[(size_t)(p ^ 1u) * D.n_tiles + tile] = tile_vacant - filled_by_plan(tile_vacant, prefix, plan);
+    }
+    if (tile < D.n_groups && threadIdx.x >= 32 && threadIdx.x < 32 + kRowWords)   // the row the next iteration adds into
+      group_row(D, p ^ 1u, tile)[threadIdx.x - 32] = 0u;
+    if (tile == 0 && threadIdx.x >= 64 && threadIdx.x < 64 + kMaxGroups / 32) D.group_mask[(p ^ 1u) * (kMaxGroups / 32) + (threadIdx.x - 64)] = 0u;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {   // the two bits the later tiles poll: "this tile has published", "this group is complete"
+      atomicOr(row + 13, 1u << (tile - tg0));
+      if (atomicAdd(row + 12, 1u) == tiles_in_group(D, g) - 1u) {
+        __threadfence();
+        atomicOr(D.group_mask + p * (kMaxGroups / 32) + g / 32, 1u << (g & 31u));
+      }
     }
   }
-  if (n_keys == 0) return;   // modes none / partition: no index array
+  const bool scatter = n_keys != 0 && (keys_read || D.write_vacant);
+  if (!scatter && !is_last) return;
+  // ---- wait for the tiles before this one: ONE thread polls the mask of complete groups (a word per 32 groups) and the
+  // mask of published tiles of the own group, with a back-off, so that a thousand waiting blocks cost L2 next to nothing;
+  // then the per-key counts of whole lower groups come from the group rows, those of the lower tiles of the own group
+  // from their own rows, all loads in flight together
+  if (threadIdx.x == 0) {
+    bool stuck = false;
+    uint32_t spins = 0;
+    const uint32_t ns = 100;   // one polling thread per block: a short, fixed pause costs L2 nothing and keeps the wake-up latency low
+    for (uint32_t w = 0; w * 32u < g && !stuck; ++w) {
+      const uint32_t want = g - w * 32u >= 32u ? 0xffffffffu : (1u << (g - w * 32u)) - 1u;
+      while ((load_acquire(D.group_mask + p * (kMaxGroups / 32) + w) & want) != want) {
+        if (++spins > kSpinLimit) { stuck = true; break; }
+        __nanosleep(ns);
+      }
+    }
+    const uint32_t want_t = (1u << (tile - tg0)) - 1u;
+    while (!stuck && (load_acquire(group_row(D, p, g) + 13) & want_t) != want_t) {
+      if (++spins > kSpinLimit) { stuck = true; break; }
+      __nanosleep(ns);
+    }
+    if (stuck) ctl->error = -9;   // CEL_ERR_INTERNAL (sticky)
+  }
   __syncthreads();
-  scatter_tile(D, sm, tile, tile_vacant);
+  {
+    const bool by_particle = D.sort_mode == 2;
+    const int n_sum = by_particle ? 12 : 8;
+    for (uint32_t i0 = 0; i0 < g + kGroupTiles; i0 += kTileThreads) {   // rows [0, g): group rows; [g, g + 32): the own group's tile rows
+      const uint32_t i = i0 + threadIdx.x;
+      uint32_t s[12];
+#pragma unroll
+      for (int j = 0; j < 12; ++j) s[j] = 0;
+      const uint32_t* row = nullptr; const uint32_t* prow = nullptr;
+      if (i < g) { row = group_row(D, p, i); prow = row + 8; }
+      else if (i < g + kGroupTiles && tg0 + (i - g) < tile) { row = D.tile_hist + (size_t)(tg0 + (i - g)) * 8; prow = D.tile_phist + (size_t)(tg0 + (i - g)) * 4; }
+      if (row) {
+        const uint4 a = __ldcg(reinterpret_cast<const uint4*>(row)), b = __ldcg(reinterpret_cast<const uint4*>(row + 4));
+        s[0] = a.x; s[1] = a.y; s[2] = a.z; s[3] = a.w; s[4] = b.x; s[5] = b.y; s[6] = b.z; s[7] = b.w;
+        if (by_particle) { const uint4 c = __ldcg(reinterpret_cast<const uint4*>(prow)); s[8] = c.x; s[9] = c.y; s[10] = c.z; s[11] = c.w; }
+      }
+#pragma unroll
+      for (int j = 0; j < 12; ++j) {
+        if (j < n_sum) {
+          const uint32_t v = __reduce_add_sync(0xffffffffu, s[j]);
+          if ((threadIdx.x & 31) == 0 && v) atomicAdd(&sm.before[j], v);
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 8) sm.base[threadIdx.x] = sm.before[D.sort_mode == 2 ? 8 + (threadIdx.x & 3) : threadIdx.x];
+  if (is_last && threadIdx.x == 0) {   // every other tile is before this one: totals = before + own
+    uint32_t act_total[8], key_total[8];
+    for (int i = 0; i < 8; ++i) {
+      act_total[i] = sm.before[i] + sm.act[i];
+      key_total[i] = D.sort_mode == 2 ? (i < 4 ? sm.before[8 + i] + sm.hist[i] : 0u) : act_total[i];
+    }
+    update_control_after_fill(D, act_total, key_total, n_keys, I - n_take, V, k, cc);
+  }
+  if (!scatter) return;
+  __syncthreads();
+  scatter_tile(D, sm, tile);
 }
 
-template <bool TRACE, int CPT>
+// ================================================================ k_push: P5 (one block per tile)
+template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
   // No "last block" here: every block forms S itself, and block 0 alone updates the control block — it writes only fields
-  // that no block of this kernel reads (n_init and iter are read through the copies k_init_fill left: n_init_fill,
-  // iter_cur). The per-tile counters are zeroed by the next k_init_fill.
+  // that no block of this kernel reads (n_init and iter are read through the copies k_fill_sort left: n_init_fill, iter_cur).
   const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
   const int32_t error = ctl->error;
   const unsigned long long I = ctl->n_init_fill;
-  uint32_t cnt[CPT];
-  load_counters<CPT>(D.tile_sec, D.n_tiles, cnt);
+  uint32_t prefix, S, tile_total;
+  tile_prefix(D, sm, D.tile_sec, tile, prefix, S, tile_total);
   if (finished) return;
   const TraceScope<K_PUSH, TRACE> trace(D, iter);
-  uint32_t prefix, S, tile_total;
-  block_prefix_total_regs<CPT>(cnt, tile, sm.scan, prefix, S, tile_total);
   const bool overflow = error != 0 || I + S > D.init_capacity;
   if (tile == 0 && threadIdx.x == 0) {
     ctl->push_total = S;
@@ -584,6 +542,7 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
     ctl->secondaries += S;
     ctl->iter = iter + 1;
   }
+  if (tile_total == 0) return;
   push_tile(D, sm, tile, I, prefix, tile_total, overflow);
 }
 
@@ -596,17 +555,38 @@ __device__ __forceinline__ bool pop_is_charged(const DeviceState& D, unsigned lo
   const unsigned long long meta = reinterpret_cast<const unsigned long long*>(D.initB + (I - 1ull - j))[3];
   return meta_ptype(meta) != P_GAMMA;
 }
+// sum of a[0..tile) and of a[0..n) by one block: the block's exclusive prefix and the grand total
+__device__ __forceinline__ void block_prefix_total(const uint32_t* a, uint32_t n, uint32_t tile, uint32_t* smem /* 18 words */,
+                                                   uint32_t& prefix, uint32_t& total) {
+  uint32_t p = 0, t = 0;
+  for (uint32_t i = threadIdx.x; i < n; i += kTileThreads) {
+    const uint32_t v = a[i];
+    t += v;
+    if (i < tile) p += v;
+  }
+  p = __reduce_add_sync(0xffffffffu, p);
+  t = __reduce_add_sync(0xffffffffu, t);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();
+  if (lane == 0) { smem[warp] = p; smem[9 + warp] = t; }
+  __syncthreads();
+  p = 0; t = 0;
+#pragma unroll
+  for (int w = 0; w < kTileThreads / 32; ++w) { p += smem[w]; t += smem[9 + w]; }
+  prefix = p; total = t;
+}
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_part_count(DeviceState D) {
   __shared__ BookSmem sm;
   pdl_prologue();
   const Control* ctl = D.ctl;
   if (ctl->finished) return;
-  const TraceScope<K_PART_COUNT, TRACE> trace(D, ctl->iter);
+  const uint32_t iter = ctl->iter;
+  const TraceScope<K_PART_COUNT, TRACE> trace(D, iter);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
-  uint32_t prefix, V;
-  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);
+  uint32_t unused, V;
+  block_prefix_total(D.tile_vac + (size_t)(iter & 1u) * D.n_tiles, D.n_tiles, 0u, sm.scan, unused, V);
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const unsigned long long j0 = (unsigned long long)tile << D.tile_shift;
   const unsigned long long j1 = min(j0 + (1ull << D.tile_shift), (unsigned long long)n_take);
@@ -628,11 +608,12 @@ __global__ void __launch_bounds__(kTileThreads) k_part_scatter(DeviceState D) {
   pdl_prologue();
   Control* ctl = D.ctl;
   if (ctl->finished) return;
-  const TraceScope<K_PART_SCATTER, TRACE> trace(D, ctl->iter);
+  const uint32_t iter = ctl->iter;
+  const TraceScope<K_PART_SCATTER, TRACE> trace(D, iter);
   const uint32_t tile = blockIdx.x;
   const unsigned long long I = ctl->n_init;
-  uint32_t prefix, V, cpre, C;
-  block_prefix_total(D.tile_vac, D.n_tiles, tile, sm.scan, prefix, V);
+  uint32_t unused, V, cpre, C;
+  block_prefix_total(D.tile_vac + (size_t)(iter & 1u) * D.n_tiles, D.n_tiles, 0u, sm.scan, unused, V);
   __syncthreads();
   block_prefix_total(D.part_cnt, D.n_tiles, tile, sm.scan, cpre, C);
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
@@ -726,8 +707,8 @@ __global__ void k_debug_math(int which, const double* in, uint32_t n, double* ou
   out[i] = which == 0 ? x * S : (x * x) * V;
 }
 
-// every slot vacant: key byte 7 (padding 0xff), meta action VACANT (state bytes are otherwise zero); the per-tile
-// vacancy counters start at the number of real slots in the tile
+// every slot vacant: key byte 7 (padding 0xff), meta action VACANT (state bytes are otherwise zero); the per-tile and
+// per-group vacancy counters start at the number of real slots
 __global__ void k_reset_state(DeviceState D) {
   const unsigned long long padded = (unsigned long long)D.n_tiles << D.tile_shift;
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < padded; i += (unsigned long long)gridDim.x * blockDim.x) {
@@ -738,11 +719,11 @@ __global__ void k_reset_state(DeviceState D) {
       RecB b; b.dx = b.dy = b.dz = 0.0; b.meta = make_meta(A_VACANT, 0, 0, -1, 0, 0);
       store_a(D.stA + i, a); store_b(D.stB + i, b);
     }
-    if (i < D.n_tiles) {
+    if (i < D.n_tiles) {   // vacancy counters of parity 0 (the fill of iteration 0 reads them); everything else in the scratch is zero
       const unsigned long long lo = i << D.tile_shift, hi = (i + 1) << D.tile_shift;
       D.tile_vac[i] = (uint32_t)(lo >= D.N ? 0ull : ((hi < D.N ? hi : (unsigned long long)D.N) - lo));
-      D.tile_sec[i] = 0;
     }
+    if (i == 0) D.ctl->iter_cur = 0xffffffffu;   // k_fill_sort forms k = iter_cur + 1 before its dependency wait
   }
 }
 

@@ -34,15 +34,16 @@ __device__ __forceinline__ void warp_aggregated_add64(unsigned long long* base, 
   }
   if (lane == leader) atomicAdd(base + cell, sum);
 }
-__device__ __forceinline__ void warp_aggregated_add32(uint32_t* base, uint32_t cell, uint32_t value) {
+// the per-tile counters of the bookkeeping kernels (vacancies created, secondaries staged): lanes of the converged set
+// that hit the same tile are combined first, so a warp issues one atomic per distinct tile. value is 0..3: the peer sums
+// are formed from two ballots. (Per-GROUP counters kept by the action kernels as well were tried and dropped: at 2^20
+// slots that is 32 addresses for the whole GPU, and same-address atomics serialise in L2 — +7 us per iteration at the
+// shower maximum.)
+__device__ __forceinline__ void warp_aggregated_add32(uint32_t* tile_cnt, uint32_t tile, uint32_t value) {
   const unsigned active = __activemask();
-  const unsigned peers = __match_any_sync(active, cell);
-  if (peers == active) {  // the common case in the sorted modes: the whole warp sits in one tile
-    const uint32_t sum = __reduce_add_sync(active, value);
-    if ((threadIdx.x & 31) == __ffs(active) - 1) atomicAdd(base + cell, sum);
-  } else {
-    atomicAdd(base + cell, value);
-  }
+  const unsigned b0 = __ballot_sync(active, value & 1u), b1 = __ballot_sync(active, value & 2u);
+  const unsigned peers = __match_any_sync(active, tile);
+  if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0) atomicAdd(tile_cnt + tile, (uint32_t)__popc(peers & b0) + 2u * (uint32_t)__popc(peers & b1));
 }
 
 // P4 (S10): q = llrint(e * 2^36) added to tally[event][bin]; bin = bin of the volume at the start of the iteration
@@ -92,20 +93,36 @@ __device__ __forceinline__ int stop_charged(const Params& P, int ptype, double& 
 
 // common epilogue: score, write the slot back, keep the dense key byte and the per-tile counters (vacancies created,
 // secondaries staged) that the scans of the next P5/P1 start from
-__device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, const Track& t, int action, int vol0, double edep,
+__device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, uint32_t k_iter, const Track& t, int action, int vol0, double edep,
                                        double eesc, int nsec, bool write_a) {
   score(D, t.event, vol0, edep, eesc);
+  const uint32_t tile = slot >> D.tile_shift;
+  if (D.reuse && action == A_VACANT && nsec >= 1) {
+    // S9-R, the general case (the interaction epilogues handle theirs without staging): the slot ends the iteration
+    // VACANT with a staged secondary — a Compton / bremsstrahlung survivor whose move then escaped or stopped. Its
+    // first staged secondary (written above by this thread) becomes the slot's track, as P1 would have made it.
+    const RecA sa = load_a(D.secA + 2ull * slot);
+    const RecB sb = load_b(D.secB + 2ull * slot);
+    if (nsec == 2) { store_a(D.secA + 2ull * slot, load_a(D.secA + 2ull * slot + 1)); store_b(D.secB + 2ull * slot, load_b(D.secB + 2ull * slot + 1)); }
+    store_a(D.stA + slot, sa);
+    store_b(D.stB + slot, sb);
+    D.akey[slot] = make_key(meta_action(sb.meta), meta_ptype(sb.meta));
+    if (nsec == 2) { D.nsec[slot] = 1; warp_aggregated_add32(D.tile_sec, tile, 1u); }
+    return;
+  }
   RecB b; b.dx = t.dx; b.dy = t.dy; b.dz = t.dz;
   b.meta = make_meta(action, t.ptype, t.vol, t.surf, t.nsteps, t.event);
   if (write_a) store_a(D.stA + slot, t.a);
   store_b(D.stB + slot, b);
   D.akey[slot] = make_key(action, t.ptype);
-  const uint32_t tile = slot >> D.tile_shift;
   if (nsec) {
     D.nsec[slot] = (uint8_t)nsec;
     warp_aggregated_add32(D.tile_sec, tile, (uint32_t)nsec);
   }
-  if (action == A_VACANT) warp_aggregated_add32(D.tile_vac, tile, 1u);
+  if (action == A_VACANT) {   // into the buffer the fill of iteration k+1 reads (parity (k+1)&1)
+    const uint32_t q = (k_iter & 1u) ^ 1u;
+    warp_aggregated_add32(D.tile_vac + (size_t)q * D.n_tiles, tile, 1u);
+  }
 }
 
 __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
@@ -121,26 +138,30 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 #define CEL_FOR_RANGE(RANGE_ID, KERNEL_ID)                                                                  \
   pdl_prologue();                                                                                           \
   const Control* ctl = D.ctl;                                                                               \
-  const uint32_t finished_ = ctl->finished;   /* the four loads are issued together: one round trip */      \
-  const uint32_t rb = ctl->rb[RANGE_ID], re = ctl->re[RANGE_ID];                                            \
+  const uint32_t finished_ = ctl->finished;   /* the loads are issued together: one round trip */           \
+  const uint32_t rb0_ = ctl->rb[RANGE_ID][0], re0_ = ctl->re[RANGE_ID][0];                                  \
+  const uint32_t rb1_ = ctl->rb[RANGE_ID][1], re1_ = ctl->re[RANGE_ID][1];                                  \
   const uint32_t k_iter = ctl->iter;                                                                        \
   if (finished_) return;                                                                                    \
   const TraceScope<KERNEL_ID, TRACE> trace(D, k_iter);                                                      \
   const Params& P = D.P;                                                                                    \
   (void)k_iter; (void)P;                                                                                    \
-  for (uint32_t tid = rb + blockIdx.x * blockDim.x + threadIdx.x; tid < re; tid += gridDim.x * blockDim.x)
+  /* the kernel's (up to) two index ranges walked as one virtual range with a grid-stride loop */         \
+  const uint32_t n0_ = re0_ - rb0_, n_ = n0_ + (re1_ - rb1_);                                               \
+  for (uint32_t i_ = blockIdx.x * blockDim.x + threadIdx.x, tid = i_ < n0_ ? rb0_ + i_ : rb1_ + (i_ - n0_); i_ < n_; \
+       i_ += gridDim.x * blockDim.x, tid = i_ < n0_ ? rb0_ + i_ : rb1_ + (i_ - n0_))
 
 __device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode == 1 || D.sort_mode == 2) ? D.indices[tid] : tid; }
 
 // S8 photoelectric: the photon's energy goes to an electron along d (or is deposited when electrons are local)
-__device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t slot, const RecA& a, const RecB& b) {
+__device__ __forceinline__ void do_photoelectric(const DeviceState& D, uint32_t slot, uint32_t k_iter, const RecA& a, const RecB& b) {
   Track t = unpack(a, b);
   double edep = 0.0;
   int nsec = 0, action = A_VACANT;
   if (D.P.electrons_local) edep += t.a.energy;
   else if (D.reuse) action = become_secondary(t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);   // only the meta word changes
   else stage_secondary(D, slot, nsec++, t, t.a.energy, t.dx, t.dy, t.dz, P_ELECTRON);
-  finish(D, slot, t, action, t.vol, edep, 0.0, nsec, false);
+  finish(D, slot, k_iter, t, action, t.vol, edep, 0.0, nsec, false);
 }
 template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
@@ -150,7 +171,7 @@ __global__ void __launch_bounds__(kBlock) k_photoelectric(DeviceState D) {
     const RecB b = load_b(D.stB + slot);
     const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     if (meta_action(b.meta) != A_PE) continue;
-    do_photoelectric(D, slot, a, b);
+    do_photoelectric(D, slot, k_iter, a, b);
   }
 }
 
@@ -169,13 +190,13 @@ __device__ __forceinline__ void do_pair(const DeviceState& D, uint32_t slot, uin
     int action;
     if (Tm >= P.cut) { stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON); action = become_secondary(t, Tm, t.dx, t.dy, t.dz, P_ELECTRON); }
     else { edep += Tm; action = become_secondary(t, Tp, t.dx, t.dy, t.dz, P_POSITRON); }
-    finish(D, slot, t, action, t.vol, edep, 0.0, nsec, true);
+    finish(D, slot, k_iter, t, action, t.vol, edep, 0.0, nsec, true);
     return;
   }
   if (Tm >= P.cut) stage_secondary(D, slot, nsec++, t, Tm, t.dx, t.dy, t.dz, P_ELECTRON);
   else edep += Tm;
   stage_secondary(D, slot, nsec++, t, Tp, t.dx, t.dy, t.dz, P_POSITRON);
-  finish(D, slot, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
+  finish(D, slot, k_iter, t, A_VACANT, t.vol, edep, 0.0, nsec, false);
 }
 template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_pair(DeviceState D) {
@@ -202,12 +223,12 @@ __device__ __forceinline__ void do_annihilation(const DeviceState& D, uint32_t s
   if (D.reuse) {   // S9-R: photon (m_e, u) takes the slot, photon (m_e, -u) is pushed
     stage_secondary(D, slot, 0, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
     const int action = become_secondary(t, kElectronMass, ux, uy, uz, P_GAMMA);
-    finish(D, slot, t, action, t.vol, 0.0, 0.0, 1, true);
+    finish(D, slot, k_iter, t, action, t.vol, 0.0, 0.0, 1, true);
     return;
   }
   stage_secondary(D, slot, 0, t, kElectronMass, ux, uy, uz, P_GAMMA);
   stage_secondary(D, slot, 1, t, kElectronMass, -ux, -uy, -uz, P_GAMMA);
-  finish(D, slot, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
+  finish(D, slot, k_iter, t, A_VACANT, t.vol, 0.0, 0.0, 2, false);
 }
 template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_annihilation(DeviceState D) {
@@ -311,7 +332,7 @@ __device__ __forceinline__ void do_photon(const DeviceState& D, uint32_t slot, u
   int action = A_MOVE_G;
   if (act == A_COMPTON) action = compton(D, slot, k_iter, t, edep, nsec);
   if (action == A_MOVE_G) action = move_photon<GEOM>(D, slot, k_iter, t, eesc);
-  finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+  finish(D, slot, k_iter, t, action, vol0, edep, eesc, nsec, true);
 }
 // (four blocks per SM = 64 registers: measured 1-3 % faster than the 80 the compiler takes unasked)
 template <int GEOM, bool TRACE>
@@ -485,7 +506,7 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
     }
   }
   if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
-  finish(D, slot, t, action, vol0, edep, eesc, nsec, true);
+  finish(D, slot, k_iter, t, action, vol0, edep, eesc, nsec, true);
 }
 // (without a field: four blocks per SM = 64 registers, the count the kernel is tuned at — 70+ registers measured 19 % slower)
 template <bool FIELD, int GEOM, bool TRACE>
@@ -512,9 +533,9 @@ __global__ void __launch_bounds__(kBlock) k_discrete(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
   const uint32_t finished_ = ctl->finished;
-  const uint32_t b_an = ctl->rb[R_ANNIH], e_an = ctl->re[R_ANNIH];
-  const uint32_t b_pe = ctl->rb[R_PE], e_pe = ctl->re[R_PE];
-  const uint32_t b_pa = ctl->rb[R_PAIR], e_pa = ctl->re[R_PAIR];
+  const uint32_t b_an = ctl->rb[R_ANNIH][0], e_an = ctl->re[R_ANNIH][0];
+  const uint32_t b_pe = ctl->rb[R_PE][0], e_pe = ctl->re[R_PE][0];
+  const uint32_t b_pa = ctl->rb[R_PAIR][0], e_pa = ctl->re[R_PAIR][0];
   const uint32_t k_iter = ctl->iter;
   if (finished_) return;
   const TraceScope<K_DISCRETE, TRACE> trace(D, k_iter);
@@ -532,7 +553,7 @@ __global__ void __launch_bounds__(kBlock) k_discrete(DeviceState D) {
       const RecB b = load_b(D.stB + slot);
       const RecA a = load_a(D.stA + slot);
       if (meta_action(b.meta) == want) {
-        if (want == A_PE) do_photoelectric(D, slot, a, b);
+        if (want == A_PE) do_photoelectric(D, slot, k_iter, a, b);
         else if (want == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
         else do_pair(D, slot, k_iter, a, b);
       }
@@ -548,7 +569,7 @@ __global__ void __launch_bounds__(kBlock) k_discrete_masked(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
   const uint32_t finished_ = ctl->finished;
-  const uint32_t re = D.sort_mode == 2 ? ctl->offsets[3] : D.N;   // by particle: the non-vacant part of the index array
+  const uint32_t re = D.N;   // (modes none / partition only: every slot, masked by the key byte)
   const uint32_t k_iter = ctl->iter;
   if (finished_) return;
   const TraceScope<K_DISCRETE, TRACE> trace(D, k_iter);
@@ -559,7 +580,7 @@ __global__ void __launch_bounds__(kBlock) k_discrete_masked(DeviceState D) {
     const RecB b = load_b(D.stB + slot);
     const RecA a = load_a(D.stA + slot);
     const int act = meta_action(b.meta);
-    if (act == A_PE) do_photoelectric(D, slot, a, b);
+    if (act == A_PE) do_photoelectric(D, slot, k_iter, a, b);
     else if (act == A_PAIR) do_pair(D, slot, k_iter, a, b);
     else if (act == A_ANNIH) do_annihilation(D, slot, k_iter, a, b);
   }

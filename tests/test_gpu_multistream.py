@@ -52,21 +52,20 @@ def test_timeline_is_ordered_and_does_not_change_results(binding):
     v = ctx.tallies_view()
     assert np.array_equal(v["fixed"], ref_fixed) and v["track_steps"] == ref["track_steps"]
     names, t = ctx.trace()
-    assert names[0] == "init_fill" and "push" in names and "discrete" in names and t.shape == (64, len(names), 2)
+    assert names[0] == "fill_sort" and "push" in names and "discrete" in names and t.shape == (64, len(names), 2)
     n = min(64, int(v["iterations"]))
     t = t.astype(np.int64)
     ran = t[:n, :, 1] > 0
-    i_fill, i_scatter, i_push = names.index("init_fill"), names.index("scatter"), names.index("push")
-    assert ran[:, i_fill].all() and ran[:, i_scatter].all() and ran[:, i_push].all()
+    i_fill, i_push = names.index("fill_sort"), names.index("push")
+    assert ran[:, i_fill].all() and ran[:, i_push].all()
     assert ran[:, names.index("charged")].all() and not ran[:, names.index("discrete")].any()   # launch per action
     assert np.all(t[:n, :, 1][ran] >= t[:n, :, 0][ran])               # end >= start
-    fill, scatter, push = t[:n, i_fill], t[:n, i_scatter], t[:n, i_push]
-    assert np.all(scatter[:, 0] >= fill[:, 1])                        # P2 after P1
-    for j in range(len(names)):                                       # actions between P2 and P5
-        if j in (i_fill, i_scatter, i_push):
+    fill, push = t[:n, i_fill], t[:n, i_push]
+    for j in range(len(names)):                                       # actions between P1 + P2 and P5
+        if j in (i_fill, i_push):
             continue
         r = ran[:, j]
-        assert np.all(t[:n, j, 0][r] >= scatter[:, 1][r]) and np.all(push[:, 0][r] >= t[:n, j, 1][r])
+        assert np.all(t[:n, j, 0][r] >= fill[:, 1][r]) and np.all(push[:, 0][r] >= t[:n, j, 1][r])
     assert np.all(fill[1:, 0] >= push[:-1, 1])                        # next iteration after the push
     # the merged launch of the three pure interactions stamps "discrete" instead of their three kernels
     ctx.set_option("merge_discrete", 1)

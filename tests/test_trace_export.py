@@ -7,7 +7,7 @@ from paper_2503_17608_b200 import trace_export as T
 
 
 def test_chrome_trace_structure():
-    names = ["init_fill", "scatter", "charged", "push"]
+    names = ["fill_sort", "scatter", "charged", "push"]
     never = np.iinfo(np.uint64).max
     stamps = np.zeros((3, 4, 2), np.uint64)
     stamps[:, :, 0] = never
@@ -21,7 +21,7 @@ def test_chrome_trace_structure():
     json.dumps(tr)                           # serialisable
     x = [e for e in tr["traceEvents"] if e["ph"] == "X"]
     assert len(x) == 6 and all(e["dur"] == 2.0 for e in x)
-    assert x[0]["ts"] == 0.0 and x[1]["ts"] == 3.0 and {e["name"] for e in x} == {"init_fill", "scatter", "push"}
+    assert x[0]["ts"] == 0.0 and x[1]["ts"] == 3.0 and {e["name"] for e in x} == {"fill_sort", "scatter", "push"}
     c = [e for e in tr["traceEvents"] if e["ph"] == "C" and e["name"] == "tracks"]
     assert [e["args"]["alive"] for e in c] == [6, 6]
     rows = T.summary_rows(names, stamps, counts, every=1)
