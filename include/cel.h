@@ -49,8 +49,9 @@ enum {
   CEL_ERR_NONFINITE = -6,     /* a non-finite energy or position was produced */
   CEL_ERR_NOT_RUN = -7,       /* cel_tallies before any cel_transport */
   CEL_ERR_MAX_ITER = -8,      /* the run did not end within max_iterations */
-  CEL_ERR_INTERNAL = -9       /* a bookkeeping block gave up waiting for the blocks before it (cannot happen when blocks
+  CEL_ERR_INTERNAL = -9,      /* a bookkeeping block gave up waiting for the blocks before it (cannot happen when blocks
                                  are dispatched in index order; reported instead of hanging) */
+  CEL_ERR_HIT_OVERFLOW = -10  /* more hit records in one batch of iterations than option hit_capacity (results invalid) */
 };
 
 /* one effective element per material (S0) */
@@ -134,6 +135,7 @@ const char* cel_last_cuda_error(cel_ctx*);
 enum { CEL_K_FILL_SORT = 0, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL_K_CHARGED, CEL_K_PUSH,
        CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
        CEL_K_DISCRETE /* photoelectric + pair + annihilation in one launch (sort by action, option merge_discrete) */,
+       CEL_K_HITS_FLUSH /* option hits = 1: the iteration's hit records streamed to the pinned host ring buffer */,
        CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
@@ -154,6 +156,34 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
  * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);
+
+/* ---- hit transfer (section 3.4) ----
+ * The paper's application hands every energy deposit ("hit") to user code on the host, so "hits must be transferred at
+ * every step iteration"; doing that with synchronous copies stalled every stream, and stream-ordered
+ * copies through pinned memory gave +10-100 %. cel_set_option("hits", m) before a transport:
+ *   m = 1: the action kernels append one cel_hit per quantised deposit (S10; the same integers the tally receives, the
+ *          escape bin included) to a device buffer; after every iteration a kernel streams the new records into one of two
+ *          pinned host ring buffers (stream-ordered, no synchronisation); after each batch of iterations the host hands
+ *          the previous batch's records to a consumer thread (the callback below), one batch behind the device.
+ *   m = 2: the "before" of PAPER.md:67: after each batch the host waits for the stream and copies the records with a
+ *          blocking cudaMemcpy on the default stream into pageable memory, then processes them inline.
+ *   m = 0: off (default; the tallies are kept on the device in any mode).
+ * "hit_capacity": records per batch of iterations (default 2^24 = 256 MB; more in one batch is CEL_ERR_HIT_OVERFLOW).
+ * "hit_tally" = 1: the library's own consumer also accumulates the records into a host tally (cel_hit_tallies), which
+ * must equal cel_tallies bit for bit (the test of the transfer). */
+typedef struct { uint32_t event; int32_t bin; uint64_t q; } cel_hit;   /* 16 bytes; q in units of 2^-36 MeV; bin n_bins = escaped */
+/* Called on the library's consumer thread (mode 1) or on the calling thread (mode 2), once per batch of iterations, in
+ * iteration order; `hits` is library-owned memory, valid during the call. */
+typedef void (*cel_hit_callback)(const cel_hit* hits, uint64_t n, void* user);
+int cel_set_hit_callback(cel_ctx*, cel_hit_callback fn, void* user);
+typedef struct {
+  uint64_t n_hits, q_sum, bytes_d2h;  /* records received by the host in the last transport, their sum, their bytes */
+  uint32_t n_events; int32_t n_bins;
+  const uint64_t* fixed;              /* option hit_tally: [n_events][n_bins+1] accumulated on the host from the records
+                                         (library-owned, valid until the next transport); NULL otherwise */
+} cel_hit_view;
+/* Synchronises the stream and waits for the consumer thread; fills *out. */
+int cel_hit_tallies(cel_ctx*, cel_hit_view* out);
 
 /* Device-side timeline (the per-iteration view of PAPER.md:81-85, fig. 2). cel_set_option("trace", n) before a
  * transport makes every kernel of the first n iterations stamp the GPU's global nanosecond timer when its first block

@@ -20,7 +20,8 @@ EXPORTS = ["cel_create", "cel_set_stream", "cel_workspace_bytes", "cel_set_works
            "cel_transport_device", "cel_tallies", "cel_destroy", "cel_strerror", "cel_last_cuda_error", "cel_set_option",
            "cel_debug_begin", "cel_debug_step", "cel_debug_read_state", "cel_debug_read_indices",
            "cel_debug_n_initializers", "cel_debug_read_initializers", "cel_debug_n_counts", "cel_debug_read_counts",
-           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace", "cel_debug_math"]
+           "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace", "cel_debug_math",
+           "cel_set_hit_callback", "cel_hit_tallies"]
 
 
 class cel_material(C.Structure):
@@ -44,6 +45,15 @@ class cel_tally_view(C.Structure):
     _fields_ = [("n_events", C.c_uint32), ("n_bins", C.c_int32), ("fixed", C.POINTER(C.c_uint64)),
                 ("track_steps", C.c_uint64), ("iterations", C.c_uint64), ("secondaries", C.c_uint64),
                 ("seconds", C.c_double), ("kernel_launches", C.c_uint64)]
+
+
+class cel_hit_view(C.Structure):
+    _fields_ = [("n_hits", C.c_uint64), ("q_sum", C.c_uint64), ("bytes_d2h", C.c_uint64), ("n_events", C.c_uint32),
+                ("n_bins", C.c_int32), ("fixed", C.POINTER(C.c_uint64))]
+
+
+HIT_DTYPE = np.dtype([("event", "<u4"), ("bin", "<i4"), ("q", "<u8")])
+HIT_CALLBACK = C.CFUNCTYPE(None, C.c_void_p, C.c_uint64, C.c_void_p)
 
 
 class CelError(RuntimeError):
@@ -94,6 +104,8 @@ def load_library():
     L.cel_kernel_name.argtypes = [C.c_int]
     L.cel_kernel_times.argtypes = [vp, vp, vp]
     L.cel_trace.argtypes = [vp, vp, vp]
+    L.cel_set_hit_callback.argtypes = [vp, HIT_CALLBACK, vp]
+    L.cel_hit_tallies.argtypes = [vp, C.POINTER(cel_hit_view)]
     _lib = L
     return L
 
@@ -206,6 +218,26 @@ class Context:
         if n.value:
             self._check(L.cel_trace(self.h, _p(out), C.byref(n)), "cel_trace")
         return [L.cel_kernel_name(i).decode() for i in range(L.cel_kernel_count())], out
+
+    def set_hit_callback(self, fn):
+        """fn(hits: numpy structured array view (HIT_DTYPE), valid during the call) or None; called per batch of iterations"""
+        if fn is None:
+            self._hit_cb = HIT_CALLBACK(0)
+        else:
+            def tramp(ptr, n, _user):
+                buf = (C.c_char * (int(n) * HIT_DTYPE.itemsize)).from_address(ptr)
+                fn(np.frombuffer(buf, dtype=HIT_DTYPE))
+            self._hit_cb = HIT_CALLBACK(tramp)
+        self._check(load_library().cel_set_hit_callback(self.h, self._hit_cb, None), "cel_set_hit_callback")
+
+    def hits_view(self):
+        v = cel_hit_view()
+        self._check(load_library().cel_hit_tallies(self.h, C.byref(v)), "cel_hit_tallies")
+        fixed = None
+        if v.fixed:
+            n = v.n_events * (v.n_bins + 1)
+            fixed = np.ctypeslib.as_array(v.fixed, shape=(n,)).reshape(v.n_events, v.n_bins + 1).copy()
+        return dict(n_hits=int(v.n_hits), q_sum=int(v.q_sum), bytes_d2h=int(v.bytes_d2h), fixed=fixed)
 
     # ---- debug / parity surface
     def begin(self, primaries, n_events):

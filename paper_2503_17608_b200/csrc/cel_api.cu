@@ -6,10 +6,13 @@
 #include "cel_physics.cuh"
 
 #include <cmath>
+#include <condition_variable>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
+#include <thread>
 #include <vector>
 
 using namespace cel;
@@ -18,6 +21,7 @@ static_assert(sizeof(cel_primary) == 64 && sizeof(PrimaryRec) == 64, "cel_primar
 static_assert(sizeof(cel_track) == 80 && sizeof(TrackRec) == 80, "cel_track layout");
 static_assert((int)K_COUNT == (int)CEL_KERNEL_COUNT && (int)K_PUSH == (int)CEL_K_PUSH && (int)K_CHARGED == (int)CEL_K_CHARGED && (int)K_FILL_SORT == (int)CEL_K_FILL_SORT, "kernel ids");
 static_assert(sizeof(RecA) == 32 && sizeof(RecB) == 32, "record layout");
+static_assert(sizeof(cel_hit) == 16 && sizeof(HitRec) == 16, "cel_hit layout");
 static_assert(sizeof(DeviceState) < 3500, "DeviceState must fit in kernel parameter space");
 
 namespace {
@@ -26,7 +30,7 @@ constexpr uint32_t kLogCapacity = 1u << 16;  // iterations whose per-action coun
 constexpr int kStatusSlots = 2;
 constexpr int kMaxKernelsPerIteration = 16;
 static_assert(CEL_ERR_INTERNAL == -9, "k_fill_sort sets -9");
-constexpr int kSideStreams = 4;
+constexpr int kSideStreams = 5;   // (the last one carries k_hits_flush beside k_push)
 
 struct HostTables {                 // per material, kept for cel_debug_table
   std::vector<double> t[5];         // compton, pe, pair, brems, range
@@ -50,9 +54,9 @@ struct cel_ctx {
   void* workspace = nullptr; uint64_t workspace_bytes = 0; bool own_workspace = false; bool laid_out = false;
   // stream-ordered scratch of the current run
   void* scratch = nullptr; void* d_tally = nullptr; void* d_prim = nullptr;
-  cudaStream_t stream = nullptr; bool own_stream = false;
-  cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
-  cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr};
+  cudaStream_t stream = nullptr; bool own_stream = false; bool stream_blocking = false;
+  cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
+  cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
@@ -69,6 +73,19 @@ struct cel_ctx {
   uint64_t launches = 0; int kernels_per_iteration = 0;
   Control last{};                   // final status of the last run
   std::string cuda_error;
+  // hit transfer (option "hits"): 1 = stream-ordered (k_hits_flush into pinned, device-mapped ring buffers
+  // after every iteration, consumed by a host thread one batch behind), 2 = the paper's "before" (a blocking cudaMemcpy
+  // on the default stream into pageable memory after every batch)
+  int hits_mode = 0; int hit_tally = 0; uint64_t hit_capacity = 1ull << 24;
+  void* d_hits = nullptr; uint64_t d_hits_cap = 0;
+  cel_hit* h_ring[2] = {nullptr, nullptr}; uint64_t h_ring_cap = 0;
+  std::vector<cel_hit> h_pageable;
+  cudaEvent_t ev_hfork = nullptr;
+  cel_hit_callback hit_cb = nullptr; void* hit_cb_user = nullptr;
+  std::thread consumer; std::mutex cmu; std::condition_variable ccv;
+  const cel_hit* job_ptr = nullptr; uint64_t job_n = 0; bool job_pending = false, consumer_stop = false, consumer_on = false;
+  uint64_t hits_total = 0, hits_qsum = 0, hits_bytes = 0;
+  std::vector<uint64_t> h_hit_tally;
   // per-kernel device timing (option "profile"): events around every launch, direct launches, one sync per batch
   int profile = 0;
   std::vector<cudaEvent_t> prof_ev;   // [batch][kMaxKernelsPerIteration + 1]
@@ -352,6 +369,7 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
     if (cudaEventCreateWithFlags(&c->ev_join[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
   }
   if (cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
+  if (cudaEventCreateWithFlags(&c->ev_hfork, cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
   if (cudaEventCreate(&c->ev_start) != cudaSuccess || cudaEventCreate(&c->ev_stop) != cudaSuccess) return fail(CEL_ERR_CUDA);
   for (int i = 0; i < kStatusSlots; ++i)
     if (cudaEventCreateWithFlags(&c->ev_batch[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
@@ -360,9 +378,61 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   return CEL_OK;
 }
 
+namespace {
+// ---------------------------------------------------------------- the host side of the hit transfer
+void consume_hits(cel_ctx* c, const cel_hit* h, uint64_t n) {   // what the "user's sensitive detector" does with a batch
+  uint64_t q = 0;
+  if (c->hit_tally) {
+    const uint64_t stride = (uint64_t)c->D.P.n_bins + 1;
+    for (uint64_t i = 0; i < n; ++i) { q += h[i].q; c->h_hit_tally[(uint64_t)h[i].event * stride + (uint64_t)h[i].bin] += h[i].q; }
+  } else {
+    for (uint64_t i = 0; i < n; ++i) q += h[i].q;
+  }
+  c->hits_total += n; c->hits_qsum += q; c->hits_bytes += n * sizeof(cel_hit);
+  if (c->hit_cb && n) c->hit_cb(h, n, c->hit_cb_user);
+}
+void consumer_main(cel_ctx* c) {
+  std::unique_lock<std::mutex> lk(c->cmu);
+  while (true) {
+    c->ccv.wait(lk, [c] { return c->job_pending || c->consumer_stop; });
+    if (c->job_pending) {
+      const cel_hit* p = c->job_ptr; const uint64_t n = c->job_n;
+      lk.unlock();
+      consume_hits(c, p, n);
+      lk.lock();
+      c->job_pending = false;
+      c->ccv.notify_all();
+    } else if (c->consumer_stop) {
+      return;
+    }
+  }
+}
+void consumer_wait_idle(cel_ctx* c) {
+  if (!c->consumer_on) return;
+  std::unique_lock<std::mutex> lk(c->cmu);
+  c->ccv.wait(lk, [c] { return !c->job_pending; });
+}
+void consumer_submit(cel_ctx* c, const cel_hit* p, uint64_t n) {
+  std::unique_lock<std::mutex> lk(c->cmu);
+  c->ccv.wait(lk, [c] { return !c->job_pending; });
+  c->job_ptr = p; c->job_n = n; c->job_pending = true;
+  c->ccv.notify_all();
+}
+void consumer_shutdown(cel_ctx* c) {
+  if (!c->consumer_on) return;
+  { std::unique_lock<std::mutex> lk(c->cmu); c->ccv.wait(lk, [c] { return !c->job_pending; }); c->consumer_stop = true; c->ccv.notify_all(); }
+  c->consumer.join();
+  c->consumer_on = false;
+}
+}  // namespace
+
 extern "C" void cel_destroy(cel_ctx* c) {
   if (!c) return;
   if (c->stream) cudaStreamSynchronize(c->stream);
+  consumer_shutdown(c);
+  if (c->d_hits) cudaFree(c->d_hits);
+  for (int i = 0; i < 2; ++i) if (c->h_ring[i]) cudaFreeHost(c->h_ring[i]);
+  if (c->ev_hfork) cudaEventDestroy(c->ev_hfork);
   for (int i = 0; i < kSideStreams; ++i) {
     if (c->side[i]) { cudaStreamSynchronize(c->side[i]); cudaStreamDestroy(c->side[i]); }
     if (c->ev_join[i]) cudaEventDestroy(c->ev_join[i]);
@@ -413,6 +483,9 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
+  else if (!std::strcmp(name, "hits")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->hits_mode = (int)v; }
+  else if (!std::strcmp(name, "hit_tally")) c->hit_tally = v ? 1 : 0;
+  else if (!std::strcmp(name, "hit_capacity")) { if (v < 1 || v > (1ll << 30)) return CEL_ERR_INVALID_ARG; c->hit_capacity = (uint64_t)v; }
   else if (!std::strcmp(name, "max_iterations")) { if (v < 1) return CEL_ERR_INVALID_ARG; c->max_iterations = v; }
   else return CEL_ERR_INVALID_ARG;
   return CEL_OK;
@@ -430,6 +503,7 @@ extern "C" const char* cel_strerror(int code) {
     case CEL_ERR_NOT_RUN: return "no transport has run";
     case CEL_ERR_MAX_ITER: return "iteration limit reached";
     case CEL_ERR_INTERNAL: return "internal error: a bookkeeping wait gave up";
+    case CEL_ERR_HIT_OVERFLOW: return "hit buffer overflow (option hit_capacity)";
     default: return "unknown error";
   }
 }
@@ -446,7 +520,7 @@ int physics_grid(const cel_ctx* c) {
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
     "fill_sort", "annihilation", "photoelectric", "pair", "photon", "charged", "push",
-    "part_count", "part_scatter", "discrete"};
+    "part_count", "part_scatter", "discrete", "hits_flush"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
@@ -465,6 +539,25 @@ void launch_chain(cel_ctx* c, K kernel, int grid, int block, cudaStream_t s) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr; cfg.numAttrs = (c->pdl && !c->profile) ? 1 : 0;
   cudaLaunchKernelEx(&cfg, kernel, c->D);
+}
+
+// P5, and beside it (option hits = 1) the transfer of the iteration's hit records to the host ring buffer
+template <bool TR>
+void enqueue_push_and_flush(cel_ctx* c, int& n) {
+  const DeviceState& D = c->D;
+  cudaStream_t s = c->stream;
+  const bool flush = c->hits_mode == 1;
+  const bool fork = flush && c->concurrent && !c->profile;
+  const int fg = c->n_sm * 4;
+  if (fork) {
+    cudaStream_t hs = c->side[kSideStreams - 1];
+    cudaEventRecord(c->ev_hfork, s); cudaStreamWaitEvent(hs, c->ev_hfork, 0);
+    k_hits_flush<TR><<<fg, kTileThreads, 0, hs>>>(D); after_launch(c, CEL_K_HITS_FLUSH, n);
+  } else if (flush) {
+    k_hits_flush<TR><<<fg, kTileThreads, 0, s>>>(D); after_launch(c, CEL_K_HITS_FLUSH, n);
+  }
+  launch_chain(c, k_push<TR>, (int)D.n_tiles, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+  if (fork) { cudaEventRecord(c->ev_join[kSideStreams - 1], c->side[kSideStreams - 1]); cudaStreamWaitEvent(s, c->ev_join[kSideStreams - 1], 0); }
 }
 
 // one step iteration = P1, P2, P3 (+P4 inside the action kernels), P5 (docs/PHYSICS_SPEC.md S1); returns the number of
@@ -500,7 +593,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     else { if (field) k_charged<true, 0, TR><<<pg, kBlock, 0, s>>>(D); else k_charged<false, 0, TR><<<pg, kBlock, 0, s>>>(D); }
     after_launch(c, CEL_K_CHARGED, n);
     if (fork) { cudaEventRecord(c->ev_join[0], c->side[0]); cudaStreamWaitEvent(s, c->ev_join[0], 0); }
-    launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+    enqueue_push_and_flush<TR>(c, n);
     return n;
   }
   // sorted by action: photon, annihilation, photoelectric, pair on one branch each (their ranges are disjoint and fixed);
@@ -532,7 +625,7 @@ int enqueue_iteration_t(cel_ctx* c) {
     cudaEventRecord(c->ev_join[i], c->side[i]);
     cudaStreamWaitEvent(s, c->ev_join[i], 0);
   }
-  launch_chain(c, k_push<TR>, tg, kTileThreads, s); after_launch(c, CEL_K_PUSH, n);
+  enqueue_push_and_flush<TR>(c, n);
   return n;
 }
 int enqueue_iteration(cel_ctx* c) { return c->trace_iters > 0 ? enqueue_iteration_t<true>(c) : enqueue_iteration_t<false>(c); }
@@ -588,6 +681,42 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
     CEL_CUDA(c, cudaStreamSynchronize(s));   // `init` is pageable host memory (measurement mode only)
     D.trace = (unsigned long long*)c->d_trace; D.trace_iters = (uint32_t)c->trace_iters;
   }
+  // hits = 2 reproduces the paper's stall: that needs a BLOCKING stream (one the default stream's
+  // synchronous copies synchronise with), so the library's own non-blocking stream is replaced by a blocking one
+  if (c->hits_mode == 2 && c->own_stream && !c->stream_blocking) {
+    CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaStreamDestroy(c->stream);
+    CEL_CUDA(c, cudaStreamCreateWithFlags(&c->stream, cudaStreamDefault));
+    c->stream_blocking = true;
+    s = c->stream;
+    if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+    if (c->graph) { cudaGraphDestroy(c->graph); c->graph = nullptr; }
+  }
+  // hit transfer: device batch buffer + (mode 1) two pinned, device-mapped host ring buffers; kept from run to run
+  D.hits = nullptr; D.hit_capacity = 0; D.host_hits[0] = D.host_hits[1] = nullptr;
+  if (c->hits_mode) {
+    if (c->d_hits_cap < c->hit_capacity) {
+      if (c->d_hits) { CEL_CUDA(c, cudaStreamSynchronize(s)); cudaFree(c->d_hits); c->d_hits = nullptr; c->d_hits_cap = 0; }
+      CEL_CUDA(c, cudaMalloc(&c->d_hits, c->hit_capacity * sizeof(cel_hit)));
+      c->d_hits_cap = c->hit_capacity;
+    }
+    if (c->hits_mode == 1 && c->h_ring_cap < c->hit_capacity) {
+      consumer_wait_idle(c);
+      for (int i = 0; i < 2; ++i) {
+        if (c->h_ring[i]) { cudaFreeHost(c->h_ring[i]); c->h_ring[i] = nullptr; }
+        CEL_CUDA(c, cudaHostAlloc((void**)&c->h_ring[i], c->hit_capacity * sizeof(cel_hit), cudaHostAllocMapped));
+      }
+      c->h_ring_cap = c->hit_capacity;
+    }
+    D.hits = (HitRec*)c->d_hits; D.hit_capacity = c->hit_capacity;
+    if (c->hits_mode == 1) {
+      for (int i = 0; i < 2; ++i) { void* dp = nullptr; CEL_CUDA(c, cudaHostGetDevicePointer(&dp, c->h_ring[i], 0)); D.host_hits[i] = (HitRec*)dp; }
+      if (!c->consumer_on) { c->consumer_stop = false; c->job_pending = false; c->consumer = std::thread(consumer_main, c); c->consumer_on = true; }
+    }
+    consumer_wait_idle(c);
+    c->hits_total = 0; c->hits_qsum = 0; c->hits_bytes = 0;
+    c->h_hit_tally.assign(c->hit_tally ? (size_t)n_events * (D.P.n_bins + 1) : 0, 0);
+  }
   CEL_CUDA(c, cudaMemsetAsync(c->scratch, 0, scratch_bytes, s));
   CEL_CUDA(c, cudaMemsetAsync(c->d_tally, 0, tally_bytes > 0 ? tally_bytes : 8, s));
   CEL_CUDA(c, cudaMemsetAsync(D.ctl, 0, sizeof(Control), s));
@@ -603,7 +732,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
   // (the stream-ordered pool hands the same scratch back run after run, so the graph of the last run is normally
   // still valid: it is kept when every baked-in argument and option is unchanged)
-  const int cfg[6] = {c->batch, c->concurrent, c->pdl, 0, c->trace_iters, c->merge_discrete};
+  const int cfg[6] = {c->batch, c->concurrent, c->pdl, c->hits_mode, c->trace_iters, c->merge_discrete};
   const bool graph_valid = c->graph_exec && std::memcmp(&c->graph_D, &D, sizeof(DeviceState)) == 0 &&
                            std::memcmp(c->graph_cfg, cfg, sizeof(cfg)) == 0;
   if (!graph_valid) {
@@ -619,10 +748,12 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
       c->prof_ev.push_back(e);
     }
   }
-  if (c->use_graph && !c->profile && !graph_valid) {
+  // (hits = 2 launches directly: a blocking default-stream copy cannot coexist with another thread's capture of a blocking stream)
+  if (c->use_graph && !c->profile && c->hits_mode != 2 && !graph_valid) {
     // one graph = one batch of iterations: a single cudaGraphLaunch per status poll keeps the host far ahead of the device
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     for (int b = 0; b < c->batch; ++b) c->kernels_per_iteration = enqueue_iteration(c);
+    if (c->hits_mode) k_hits_batch_end<<<1, 1, 0, s>>>(c->D);
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
     CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
     std::memcpy(&c->graph_D, &D, sizeof(DeviceState));
@@ -678,24 +809,44 @@ int run_loop(cel_ctx* c) {
   int rc = CEL_OK;
   while (true) {
     int per_iter = c->kernels_per_iteration;
-    if (c->graph_exec && c->use_graph && !c->profile) {
+    // hits, mode 1: the batch about to be enqueued streams into the ring buffer the consumer read two batches ago
+    if (c->hits_mode == 1) consumer_wait_idle(c);
+    if (c->graph_exec && c->use_graph && !c->profile && c->hits_mode != 2) {
       CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s));
-      c->launches += (uint64_t)c->kernels_per_iteration * c->batch;
+      c->launches += (uint64_t)c->kernels_per_iteration * c->batch + (c->hits_mode ? 1 : 0);
     } else {
       for (int b = 0; b < c->batch; ++b) {
         c->prof_b = b;
         per_iter = enqueue_iteration(c); c->launches += per_iter;
       }
+      if (c->hits_mode) { k_hits_batch_end<<<1, 1, 0, s>>>(c->D); c->launches += 1; }
     }
     c->prof_b = 0;
     enqueued += c->batch;
     if (c->profile) { int prc = collect_profile(c, c->batch, per_iter); if (prc != CEL_OK) return prc; }
+    if (c->hits_mode == 2) {
+      // the paper's "before": wait for the batch, then a blocking copy on the default stream into pageable
+      // memory — a device-wide synchronisation for every stream that is not non-blocking — and process the hits inline
+      CEL_CUDA(c, cudaStreamSynchronize(s));
+      Control st;
+      CEL_CUDA(c, cudaMemcpy(&st, c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost));
+      if (st.hits_in_batch) {
+        if (c->h_pageable.size() < st.hits_in_batch) c->h_pageable.resize(st.hits_in_batch);
+        CEL_CUDA(c, cudaMemcpy(c->h_pageable.data(), c->d_hits, st.hits_in_batch * sizeof(cel_hit), cudaMemcpyDeviceToHost));
+        consume_hits(c, c->h_pageable.data(), st.hits_in_batch);
+      }
+      if (st.error != 0) { rc = st.error; break; }
+      if (st.finished) break;
+      if (enqueued >= c->max_iterations) { rc = CEL_ERR_MAX_ITER; break; }
+      continue;
+    }
     CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
     CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
     if (have_prev) {
       const int prev = slot ^ 1;
       CEL_CUDA(c, cudaEventSynchronize(c->ev_batch[prev]));
       const Control& st = c->h_status[prev];
+      if (c->hits_mode == 1 && st.hits_in_batch) consumer_submit(c, c->h_ring[st.hits_buf & 1u], st.hits_in_batch);
       if (st.error != 0) { rc = st.error; break; }
       if (st.finished) break;
     }
@@ -746,6 +897,24 @@ extern "C" int cel_tallies(cel_ctx* c, cel_tally_view* out) {
   out->seconds = (cudaEventElapsedTime(&ms, c->ev_start, c->ev_stop) == cudaSuccess) ? ms * 1e-3 : 0.0;
   out->kernel_launches = c->launches;
   if (c->last.error != 0) return c->last.error;
+  return c->run_error;
+}
+
+extern "C" int cel_set_hit_callback(cel_ctx* c, cel_hit_callback fn, void* user) {
+  if (!c) return CEL_ERR_INVALID_ARG;
+  consumer_wait_idle(c);
+  c->hit_cb = fn; c->hit_cb_user = user;
+  return CEL_OK;
+}
+
+extern "C" int cel_hit_tallies(cel_ctx* c, cel_hit_view* out) {
+  if (!c || !out) return CEL_ERR_INVALID_ARG;
+  if (!c->ran) return CEL_ERR_NOT_RUN;
+  CEL_CUDA(c, cudaStreamSynchronize(c->stream));
+  consumer_wait_idle(c);
+  out->n_hits = c->hits_total; out->q_sum = c->hits_qsum; out->bytes_d2h = c->hits_bytes;
+  out->n_events = c->D.n_events; out->n_bins = c->D.P.n_bins;
+  out->fixed = c->h_hit_tally.empty() ? nullptr : c->h_hit_tally.data();
   return c->run_error;
 }
 

@@ -121,7 +121,17 @@ struct Control {
   unsigned long long n_init_fill;   // I after the fill of this iteration (= n_init until k_push adds S)
   uint32_t iter_cur;                // k of the running iteration, a copy k_push may read while its block 0 bumps iter
   uint32_t part_charged;            // sort mode 3: charged initializers among the n_take popped in this iteration
+  // hit transfer (option "hits")
+  unsigned long long n_hits;        // hit records appended to the device batch buffer since the batch began
+  unsigned long long hits_mark[2];  // [k&1] = records already streamed to the host when iteration k's flush starts
+  unsigned long long hits_in_batch; // set by k_hits_batch_end: records of the batch that just ended ...
+  uint32_t hits_buf;                // ... and the host ring buffer (0/1) they were streamed into
+  uint32_t hits_cur;                // the host ring buffer the running batch streams into
 };
+
+// one hit = one quantised deposit of one track in one iteration (S10): what the paper's application copies to the host
+// at every step iteration for the user's sensitive detectors. = cel_hit of include/cel.h, 16 bytes.
+struct HitRec { uint32_t event; int32_t bin; unsigned long long q; };
 
 // everything a kernel needs; passed by value (fits in the 4 KB parameter space)
 struct DeviceState {
@@ -156,6 +166,10 @@ struct DeviceState {
   uint32_t* group_rows;   // [2][kMaxGroups][kRowWords] group histograms + arrival counters, double-buffered by iteration parity
   uint32_t* group_mask;   // [2][kMaxGroups / 32] bit g = every tile of group g has published its rows of this iteration
   uint32_t* part_cnt;     // [n_tiles] sort mode 3: charged pops per tile-sized chunk of the popped segment
+  // hit transfer (option "hits"): device batch buffer the action kernels append to, the two pinned host ring buffers
+  // (device-mapped) k_hits_flush streams it into; nullptr = off
+  HitRec* hits; unsigned long long hit_capacity;
+  HitRec* host_hits[2];
   // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
   // in / last warp out of every kernel of every iteration; nullptr = off
   unsigned long long* trace;
@@ -164,7 +178,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_FILL_SORT = 0, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_COUNT };
+enum KernelId : int { K_FILL_SORT = 0, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_HITS_FLUSH, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;

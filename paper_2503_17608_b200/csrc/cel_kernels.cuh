@@ -642,6 +642,41 @@ __global__ void __launch_bounds__(kTileThreads) k_part_scatter(DeviceState D) {
   }
 }
 
+// ================================================================ hit transfer (option "hits"; section 3.4)
+// "Hits must be transferred at every step iteration": after the action kernels of iteration k, k_hits_flush
+// streams the records they appended, d_hits[mark, n_hits), into the pinned host ring buffer of the running batch at the
+// same offsets — plain coalesced 16-byte stores to device-mapped pinned memory, stream-ordered, no host involvement and no
+// synchronisation of any kind. It runs beside k_push. The marks are double-buffered by iteration parity so
+// that no block reads a field another block of the same launch writes.
+template <bool TRACE>
+__global__ void __launch_bounds__(kTileThreads) k_hits_flush(DeviceState D) {
+  Control* ctl = D.ctl;
+  const uint32_t k = ctl->iter_cur;
+  if (ctl->finished) return;
+  const TraceScope<K_HITS_FLUSH, TRACE> trace(D, k);
+  const unsigned long long lo = ctl->hits_mark[k & 1u];
+  unsigned long long hi = ctl->n_hits;
+  if (hi > D.hit_capacity) hi = D.hit_capacity;
+  HitRec* dst = D.host_hits[ctl->hits_cur & 1u];
+  for (unsigned long long i = lo + blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < hi; i += (unsigned long long)gridDim.x * blockDim.x) {
+    unsigned long long a, b;
+    asm volatile("ld.global.v2.b64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(D.hits + i));
+    asm volatile("st.global.v2.b64 [%0], {%1,%2};" ::"l"(dst + i), "l"(a), "l"(b) : "memory");
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) ctl->hits_mark[(k & 1u) ^ 1u] = hi;
+}
+// end of a batch of iterations: publish the batch's record count and ring buffer in the control block (the host reads
+// them from its asynchronous status copy), start the next batch's records at offset 0 of the other ring buffer
+__global__ void k_hits_batch_end(DeviceState D) {
+  Control* ctl = D.ctl;
+  unsigned long long n = ctl->n_hits;
+  if (n > D.hit_capacity) n = D.hit_capacity;
+  ctl->hits_in_batch = n;
+  ctl->hits_buf = ctl->hits_cur;
+  ctl->hits_cur ^= 1u;
+  ctl->n_hits = 0; ctl->hits_mark[0] = 0; ctl->hits_mark[1] = 0;
+}
+
 // ================================================================ loading, reset, debug helpers
 struct PrimaryRec { uint32_t event; int32_t ptype; double energy; double pos[3]; double dir[3]; };  // = cel_primary, 64 B
 struct TrackRec { double pos[3]; double dir[3]; double energy; uint32_t event, nsteps; int32_t vol, surf, ptype, action; };  // = cel_track

@@ -46,16 +46,41 @@ __device__ __forceinline__ void warp_aggregated_add32(uint32_t* tile_cnt, uint32
   if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0) atomicAdd(tile_cnt + tile, (uint32_t)__popc(peers & b0) + 2u * (uint32_t)__popc(peers & b1));
 }
 
+// Hit records (option "hits"): the lanes of the converged set that have a hit reserve their places in the
+// device batch buffer with ONE atomic (warp-aggregated), then write their 16-byte records; overflow is a sticky error.
+__device__ __forceinline__ void append_hit(const DeviceState& D, bool has, uint32_t event, int bin, unsigned long long q) {
+  const unsigned active = __activemask();
+  const unsigned m = __ballot_sync(active, has);
+  if (m == 0) return;
+  const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+  unsigned long long base = 0;
+  if (lane == leader) base = atomicAdd(&D.ctl->n_hits, (unsigned long long)__popc(m));
+  base = __shfl_sync(active, base, leader);
+  if (has) {
+    const unsigned long long at = base + (unsigned long long)__popc(m & ((1u << lane) - 1u));
+    if (at < D.hit_capacity) {
+      asm volatile("st.global.v2.b64 [%0], {%1,%2};" ::"l"(D.hits + at), "l"((unsigned long long)event | ((unsigned long long)(uint32_t)bin << 32)), "l"(q) : "memory");
+    } else {
+      D.ctl->error = -10;   // CEL_ERR_HIT_OVERFLOW (sticky)
+    }
+  }
+}
+
 // P4 (S10): q = llrint(e * 2^36) added to tally[event][bin]; bin = bin of the volume at the start of the iteration
 __device__ __forceinline__ void score(const DeviceState& D, uint32_t event, int vol0, double edep, double eesc) {
   const unsigned long long row = (unsigned long long)event * (unsigned long long)(D.P.n_bins + 1);
   const long long q_dep = quantise(edep);
+  int bin = -1;
   if (q_dep != 0) {
-    const int bin = __ldg(D.P.vol_bin + vol0);
+    bin = __ldg(D.P.vol_bin + vol0);
     if (bin >= 0) warp_aggregated_add64(D.tally, row + (unsigned long long)bin, (unsigned long long)q_dep);
   }
   const long long q_esc = quantise(eesc);
   if (q_esc != 0) warp_aggregated_add64(D.tally, row + (unsigned long long)D.P.n_bins, (unsigned long long)q_esc);
+  if (D.hits != nullptr) {   // the same integers, as records for the host (a measurement / application mode)
+    append_hit(D, q_dep != 0 && bin >= 0, event, bin, (unsigned long long)q_dep);
+    append_hit(D, q_esc != 0, event, D.P.n_bins, (unsigned long long)q_esc);
+  }
 }
 
 // ---------------------------------------------------------------- the registers of one track

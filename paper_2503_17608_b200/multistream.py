@@ -65,3 +65,48 @@ class MultiStream:
         for c, _, _, _ in self.parts:
             c.close()
         self.parts = []
+
+
+def main():
+    """measurement of PAPER.md section 3.4 on one GPU: K event-parallel contexts, with the hit transfer off, stream-ordered
+    (hits = 1) and synchronous (hits = 2, the paper's "before"); wall clock of the whole transport, best of `--repeat`"""
+    import argparse
+    import time
+    import torch
+    from . import workloads as W
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--workload", default="config2", choices=["config2", "config3", "config4", "config5"])
+    ap.add_argument("--streams", default="1,2,4,8,16")
+    ap.add_argument("--hits", default="0,1,2")
+    ap.add_argument("--sort-mode", type=int, default=1)
+    ap.add_argument("--repeat", type=int, default=3)
+    args = ap.parse_args()
+    assert torch.cuda.is_available(), "needs a CUDA device"
+    w = getattr(W, args.workload)(sort_mode=args.sort_mode)
+    print(f"# {w.name}: {w.n_events} events, {w.n_slots} slots in total, sort mode {args.sort_mode}; ms per transport (wall clock, best of {args.repeat})")
+    print("# streams | " + " | ".join(f"hits={h}" for h in args.hits.split(",")) + " | hit records, MB to the host")
+    for k in [int(x) for x in args.streams.split(",")]:
+        cells, info = [], ""
+        for h in [int(x) for x in args.hits.split(",")]:
+            opts = {"hits": h, "hit_capacity": max(1 << 20, 16 * (w.n_slots // k))} if h else {}
+            ms = MultiStream(w, k, options=opts)
+            ms.transport()                                      # warm-up (graph capture, pinned allocations)
+            best = 1e30
+            for _ in range(args.repeat):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                ms.transport()
+                if h:
+                    hv = [c.hits_view() for c, _, n, _ in ms.parts if n]     # waits for the consumers
+                else:
+                    ms.views()
+                best = min(best, time.perf_counter() - t0)
+            if h:
+                info = f"{sum(v['n_hits'] for v in hv)} records, {sum(v['bytes_d2h'] for v in hv) / 1e6:.0f} MB"
+            cells.append(f"{best * 1e3:8.2f}")
+            ms.close()
+        print(f"{k:9d} | " + " | ".join(cells) + " | " + info, flush=True)
+
+
+if __name__ == "__main__":
+    main()
