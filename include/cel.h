@@ -45,8 +45,8 @@ enum {
   CEL_ERR_CUDA = -2,          /* a CUDA runtime call failed (cel_last_cuda_error gives the text) */
   CEL_ERR_OOM = -3,           /* device or pinned allocation failed */
   CEL_ERR_INIT_OVERFLOW = -4, /* initializer stack exceeded init_capacity (S9); results invalid */
-  CEL_ERR_TALLY_OVERFLOW = -5,
-  CEL_ERR_NONFINITE = -6,     /* a non-finite energy or position was produced */
+  CEL_ERR_TALLY_OVERFLOW = -5,/* a single deposit of 2^63 quanta (2^27 MeV) or more, or a negative one (S10); sticky, results invalid */
+  CEL_ERR_NONFINITE = -6,     /* a non-finite energy, position or direction: in a device-resident primary, or produced by a step; sticky */
   CEL_ERR_NOT_RUN = -7,       /* cel_tallies before any cel_transport */
   CEL_ERR_MAX_ITER = -8,      /* the run did not end within max_iterations */
   CEL_ERR_INTERNAL = -9,      /* a bookkeeping block gave up waiting for the blocks before it (cannot happen when blocks
@@ -74,7 +74,7 @@ typedef struct {
   int enable_pair, enable_brems, enable_msc, enable_eloss, enable_annihilation;
   int electrons_local;     /* 1 = every electron is deposited where it is born (config 1) */
   int max_substeps;        /* field substeps per iteration, 10 in the paper */
-  uint32_t max_steps_per_track; /* looper kill (S7.6) */
+  uint32_t max_steps_per_track; /* looper kill (S7.6); 1..65535 (the step count is a 16-bit field of the slot state) */
   uint64_t init_capacity;  /* initializer stack capacity; 0 = max(8 n_slots, 2^24) */
 } cel_physics;
 
@@ -119,7 +119,9 @@ int cel_set_workspace(cel_ctx*, void* dptr, uint64_t bytes);
 int cel_transport(cel_ctx*, const cel_primary* primaries, uint64_t n_primaries, uint32_t n_events);
 
 /* Same, but the primaries are already resident in DEVICE memory as n_primaries packed cel_primary records
- * (validated by the caller); used to time the path with inputs in HBM. */
+ * (checked on the device as they are loaded: a bad event / type / volume / direction is CEL_ERR_INVALID_ARG, a non-finite or
+ * non-positive energy CEL_ERR_NONFINITE, reported by the transport or the next cel_tallies); used to time the path with
+ * inputs in HBM. n_events <= 2^24 in every transport call (the event id is a 24-bit field of the slot state). */
 int cel_transport_device(cel_ctx*, const void* d_primaries, uint64_t n_primaries, uint32_t n_events);
 
 /* Synchronises the stream, copies the integer tallies to pinned host memory and fills *out. */

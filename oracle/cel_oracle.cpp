@@ -20,7 +20,7 @@
 // Parity unpinned (no external truth exists): per-layer shower profiles of the simplified
 // physics (configs 2-5) — sanity checks only (shower maximum, containment).
 //
-// Build: g++ -O2 -ffp-contract=off -std=c++17 -shared -fPIC (see oracle/build.py).
+// Build: g++ -O2 -ffp-contract=off -fopenmp -std=c++17 -shared -fPIC (see oracle/build.py).
 
 #include <cmath>
 #include <cstdint>
@@ -379,6 +379,7 @@ struct Oracle {
   uint32_t iter;
   uint64_t track_steps, iterations, secondaries;
   int error;
+  int n_threads = 1;   // host threads of the per-slot phases (orc_set_threads)
 };
 
 int locate_primary(const Geometry& g, const double pos[3], const double dir[3]) {
@@ -769,13 +770,18 @@ void phases_after_reindex(Oracle& o) {
     const OrcTrack& t = o.tracks[s];
     o.stage[s].bin = (t.action != VACANT) ? o.geo.vol_bin[t.vol] : -1;
   }
-  // P3i: every kernel runs over its range of the sorted index array; the result does not depend on the order
+  // P3i: every kernel runs over its range of the sorted index array; the result does not depend on the order.
+  // (The two per-slot loops touch only their own slot's track and staging and draw from counter-based streams, so they
+  // may run on several host threads — orc_set_threads, OpenMP — with bit-identical results; init, reindex, score and
+  // push stay serial. The default is one thread.)
+#pragma omp parallel for schedule(static) num_threads(o.n_threads) if (o.n_threads > 1)
   for (uint64_t tid = 0; tid < o.n_slots; ++tid) {
     uint32_t slot = o.indices[tid];
     int a = o.tracks[slot].action;
     if (a == PE || a == PAIR || a == COMPTON || a == BREMS || a == ANNIH) interact_slot(o, slot);
   }
   // P3m
+#pragma omp parallel for schedule(dynamic, 256) num_threads(o.n_threads) if (o.n_threads > 1)
   for (uint64_t tid = 0; tid < o.n_slots; ++tid) {
     uint32_t slot = o.indices[tid];
     int a = o.tracks[slot].action;
@@ -821,6 +827,9 @@ void* orc_create(const OrcGeometry* g, const OrcMaterial* mats, int n_mats, cons
 }
 
 void orc_destroy(void* h) { delete (Oracle*)h; }
+
+// host threads used by the per-slot phases P3i / P3m (>= 1); results do not depend on it
+void orc_set_threads(void* h, int n) { ((Oracle*)h)->n_threads = n < 1 ? 1 : n; }
 
 int orc_n_bins(void* h) { return ((Oracle*)h)->n_bins; }
 

@@ -52,6 +52,7 @@ def lib():
         L.orc_create.argtypes = [C.POINTER(_Geometry), C.POINTER(_Material), C.c_int, C.POINTER(_Physics), C.c_uint64, C.c_int]
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_n_bins.argtypes = [C.c_void_p]
+        L.orc_set_threads.argtypes = [C.c_void_p, C.c_int]
         L.orc_begin.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint32]
         L.orc_step.argtypes = [C.c_void_p]
         L.orc_phase_init.argtypes = [C.c_void_p]
@@ -159,6 +160,10 @@ class Oracle:
         self.h = L.orc_create(C.byref(g), mats, len(materials), C.byref(ph), self.n_slots, int(sort_mode))
         self.n_bins = L.orc_n_bins(self.h)
         self.n_events = 0
+
+    def set_threads(self, n):
+        """host threads of the per-slot phases (OpenMP); results are bit-identical for any n"""
+        lib().orc_set_threads(self.h, int(n))
 
     def close(self):
         if self.h:

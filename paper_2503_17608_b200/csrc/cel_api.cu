@@ -58,6 +58,7 @@ struct cel_ctx {
   cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
   cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
+  int grid_cap = 8;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
@@ -288,6 +289,7 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   }
   if (g->kind == CEL_GEOM_CYL && g->bounds[0] != 0.0) return CEL_ERR_INVALID_ARG;
   if (!(ph->cut_MeV > 0.0) || ph->max_substeps < 1) return CEL_ERR_INVALID_ARG;
+  if (ph->max_steps_per_track < 1 || ph->max_steps_per_track > 65535u) return CEL_ERR_INVALID_ARG;   // the step count is a 16-bit field of the slot's meta word
   for (int i = 0; i < n_mats; ++i)
     if (!(mats[i].density_g_cm3 > 0.0) || !(mats[i].Z > 0.0) || !(mats[i].A > 0.0)) return CEL_ERR_INVALID_ARG;
 
@@ -483,6 +485,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
+  else if (!std::strcmp(name, "grid_cap")) { if (v < 1 || v > 32) return CEL_ERR_INVALID_ARG; c->grid_cap = (int)v; }
   else if (!std::strcmp(name, "hits")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->hits_mode = (int)v; }
   else if (!std::strcmp(name, "hit_tally")) c->hit_tally = v ? 1 : 0;
   else if (!std::strcmp(name, "hit_capacity")) { if (v < 1 || v > (1ll << 30)) return CEL_ERR_INVALID_ARG; c->hit_capacity = (uint64_t)v; }
@@ -514,7 +517,7 @@ namespace {
 
 int physics_grid(const cel_ctx* c) {
   const uint64_t need = (c->n_slots + kBlock - 1) / kBlock;
-  const uint64_t cap = (uint64_t)c->n_sm * 8;
+  const uint64_t cap = (uint64_t)c->n_sm * (uint64_t)c->grid_cap;
   return (int)(need < cap ? need : cap);
 }
 
@@ -732,7 +735,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   // the iteration as a CUDA graph: kernel arguments (scratch and tally pointers) are baked in, so re-capture per run
   // (the stream-ordered pool hands the same scratch back run after run, so the graph of the last run is normally
   // still valid: it is kept when every baked-in argument and option is unchanged)
-  const int cfg[6] = {c->batch, c->concurrent, c->pdl, c->hits_mode, c->trace_iters, c->merge_discrete};
+  const int cfg[6] = {c->batch, c->concurrent + 2 * c->grid_cap, c->pdl, c->hits_mode, c->trace_iters, c->merge_discrete};
   const bool graph_valid = c->graph_exec && std::memcmp(&c->graph_D, &D, sizeof(DeviceState)) == 0 &&
                            std::memcmp(c->graph_cfg, cfg, sizeof(cfg)) == 0;
   if (!graph_valid) {
@@ -863,7 +866,7 @@ int run_loop(cel_ctx* c) {
 }  // namespace
 
 extern "C" int cel_transport(cel_ctx* c, const cel_primary* primaries, uint64_t n, uint32_t n_events) {
-  if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  if (!c || (!primaries && n) || n_events < 1 || n_events > (1u << 24) || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
   int rc = validate_primaries(c, primaries, n, n_events);
   if (rc != CEL_OK) return rc;
   if ((rc = prepare_run(c, n_events, false)) != CEL_OK) return rc;
@@ -872,7 +875,7 @@ extern "C" int cel_transport(cel_ctx* c, const cel_primary* primaries, uint64_t 
 }
 
 extern "C" int cel_transport_device(cel_ctx* c, const void* d_primaries, uint64_t n, uint32_t n_events) {
-  if (!c || (!d_primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  if (!c || (!d_primaries && n) || n_events < 1 || n_events > (1u << 24) || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
   int rc = prepare_run(c, n_events, false);
   if (rc != CEL_OK) return rc;
   k_load_primaries<<<c->n_sm, 256, 0, c->stream>>>(c->D, (const PrimaryRec*)d_primaries, n);
@@ -939,7 +942,7 @@ extern "C" int cel_kernel_times(cel_ctx* c, double* ms_out, uint64_t* launches_o
 
 // ================================================================ debug / parity surface (synchronous)
 extern "C" int cel_debug_begin(cel_ctx* c, const cel_primary* primaries, uint64_t n, uint32_t n_events) {
-  if (!c || (!primaries && n) || n_events < 1 || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
+  if (!c || (!primaries && n) || n_events < 1 || n_events > (1u << 24) || n > c->D.init_capacity) return CEL_ERR_INVALID_ARG;
   int rc = validate_primaries(c, primaries, n, n_events);
   if (rc != CEL_OK) return rc;
   if ((rc = prepare_run(c, n_events, true)) != CEL_OK) return rc;

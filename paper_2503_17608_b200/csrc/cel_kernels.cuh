@@ -702,7 +702,13 @@ __global__ void k_load_primaries(DeviceState D, const PrimaryRec* prim, unsigned
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n; i += (unsigned long long)gridDim.x * blockDim.x) {
     const PrimaryRec p = prim[i];
     int vol = locate_volume(D.P, p.pos[0], p.pos[1], p.pos[2], p.dir[2]);
-    if (vol < 0 || p.event >= D.n_events || p.ptype < 0 || p.ptype > 2) { D.ctl->error = -1; vol = 0; }
+    // the checks validate_primaries makes on the host path (cel_transport), for primaries that are already on the device
+    const double n2 = p.dir[0] * p.dir[0] + p.dir[1] * p.dir[1] + p.dir[2] * p.dir[2];
+    bool bad = vol < 0 || p.event >= D.n_events || p.event >= (1u << 24) || p.ptype < 0 || p.ptype > 2 || !(fabs(n2 - 1.0) <= 1e-12);
+    if (D.P.geom_kind == 0) bad = bad || fabs(p.pos[0]) > D.P.half_x || fabs(p.pos[1]) > D.P.half_y;
+    else bad = bad || fabs(p.pos[2]) > D.P.half_z;
+    if (!(p.energy > 0.0) || !isfinite(p.energy) || !isfinite((p.pos[0] + p.pos[1]) + p.pos[2])) { D.ctl->error = -6; vol = vol < 0 ? 0 : vol; }   // CEL_ERR_NONFINITE
+    else if (bad) { D.ctl->error = -1; vol = vol < 0 ? 0 : vol; }
     RecA a; a.x = p.pos[0]; a.y = p.pos[1]; a.z = p.pos[2]; a.energy = p.energy;
     RecB b; b.dx = p.dir[0]; b.dy = p.dir[1]; b.dz = p.dir[2];
     b.meta = make_meta(p.ptype == P_GAMMA ? A_MOVE_G : A_MOVE_C, p.ptype, vol, -1, 0, p.event);

@@ -77,6 +77,9 @@ __device__ __forceinline__ void score(const DeviceState& D, uint32_t event, int 
   }
   const long long q_esc = quantise(eesc);
   if (q_esc != 0) warp_aggregated_add64(D.tally, row + (unsigned long long)D.P.n_bins, (unsigned long long)q_esc);
+  // S10: a single deposit of 2^63 quanta = 2^27 MeV or more (the conversion saturates), a negative or a non-finite
+  // deposit: sticky CEL_ERR_TALLY_OVERFLOW (deposits are never negative in this physics)
+  if (!(edep < 134217728.0) || !(eesc < 134217728.0) || (q_dep | q_esc) < 0) D.ctl->error = -5;
   if (D.hits != nullptr) {   // the same integers, as records for the host (a measurement / application mode)
     append_hit(D, q_dep != 0 && bin >= 0, event, bin, (unsigned long long)q_dep);
     append_hit(D, q_esc != 0, event, D.P.n_bins, (unsigned long long)q_esc);
@@ -121,6 +124,8 @@ __device__ __forceinline__ int stop_charged(const Params& P, int ptype, double& 
 __device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, uint32_t k_iter, const Track& t, int action, int vol0, double edep,
                                        double eesc, int nsec, bool write_a) {
   score(D, t.event, vol0, edep, eesc);
+  // a non-finite energy, position or direction must not go on (grid_locate would send a NaN to cell 0): sticky CEL_ERR_NONFINITE
+  if (!isfinite(((t.a.x + t.a.y) + (t.a.z + t.a.energy)) + ((t.dx + t.dy) + t.dz))) D.ctl->error = -6;
   const uint32_t tile = slot >> D.tile_shift;
   if (D.reuse && action == A_VACANT && nsec >= 1) {
     // S9-R, the general case (the interaction epilogues handle theirs without staging): the slot ends the iteration
@@ -163,7 +168,8 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
 #define CEL_FOR_RANGE(RANGE_ID, KERNEL_ID)                                                                  \
   pdl_prologue();                                                                                           \
   const Control* ctl = D.ctl;                                                                               \
-  const uint32_t finished_ = ctl->finished;   /* the loads are issued together: one round trip */           \
+  /* (a sticky error also stops the action kernels: a bad device-resident primary must not be stepped) */  \
+  const uint32_t finished_ = ctl->finished | (uint32_t)ctl->error;   /* the loads are issued together: one round trip */ \
   const uint32_t rb0_ = ctl->rb[RANGE_ID][0], re0_ = ctl->re[RANGE_ID][0];                                  \
   const uint32_t rb1_ = ctl->rb[RANGE_ID][1], re1_ = ctl->re[RANGE_ID][1];                                  \
   const uint32_t k_iter = ctl->iter;                                                                        \
@@ -434,28 +440,29 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
       if (n == P.max_substeps) break;  // paused: the remainder is re-sampled next iteration
       double h = fmin(remaining, h_max);
       const HelixFrame F = helix_frame(P, t.dx, t.dy, t.dz);
-      double nx, ny, nz, ndx, ndy, ndz, l, chx, chy, chz, tb;
+      // The chord c = pos(h) - pos is used UN-normalised: the distance to the boundary along it then comes out in units of
+      // the chord (f = t / |c| of S7.3 directly), "t <= |c|" is "f <= 1", and the sign tests of the dip rule and of the
+      // crossing do not care about the scale — no square root and no three divisions per substep (the same reals as S7.3,
+      // rounded differently in the last place)
+      double nx, ny, nz, ndx, ndy, ndz, cx, cy, cz, fb;
       int which;
       for (int halvings = 0;; ++halvings) {
         helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, h, nx, ny, nz, ndx, ndy, ndz);
-        const double cx = nx - t.a.x, cy = ny - t.a.y, cz = nz - t.a.z;
-        l = sqrt(cx * cx + cy * cy + cz * cz);
-        chx = cx / l; chy = cy / l; chz = cz / l;
-        tb = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, chx, chy, chz, t.vol, t.surf, l, which);
+        cx = nx - t.a.x; cy = ny - t.a.y; cz = nz - t.a.z;
+        fb = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, cx, cy, cz, t.vol, t.surf, 1.0, which);
         // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
-        if (tb == 0.0 && halvings < kMaxDipHalvings &&
-            tangent_points_inward(P, t.a.x, t.a.y, t.dx, t.dy, t.dz, chx, chy, chz, which)) { h *= 0.5; continue; }
+        if (fb == 0.0 && halvings < kMaxDipHalvings &&
+            tangent_points_inward(P, t.a.x, t.a.y, t.dx, t.dy, t.dz, cx, cy, cz, which)) { h *= 0.5; continue; }
         break;
       }
-      if (tb <= l) {
-        const double f = tb / l;
+      if (fb <= 1.0) {
         double fx, fy, fz, fdx, fdy, fdz;
-        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, f * h, fx, fy, fz, fdx, fdy, fdz);
-        t.a.x += tb * chx; t.a.y += tb * chy; t.a.z += tb * chz;
+        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, fb * h, fx, fy, fz, fdx, fdy, fdz);
+        t.a.x += fb * cx; t.a.y += fb * cy; t.a.z += fb * cz;
         normalise3(fdx, fdy, fdz);
         t.dx = fdx; t.dy = fdy; t.dz = fdz;
-        travelled += f * h;
-        escaped = cross_boundary<GEOM>(P, t.a.z, chz, t.vol, t.surf, which);
+        travelled += fb * h;
+        escaped = cross_boundary<GEOM>(P, t.a.z, cz, t.vol, t.surf, which);
         break;
       }
       normalise3(ndx, ndy, ndz);
@@ -533,9 +540,10 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
   if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
   finish(D, slot, k_iter, t, action, vol0, edep, eesc, nsec, true);
 }
-// (without a field: four blocks per SM = 64 registers, the count the kernel is tuned at — 70+ registers measured 19 % slower)
+// (without a field: four blocks per SM = 64 registers, the count the kernel is tuned at — 70+ registers measured 19 % slower;
+// with a field: three blocks per SM = 85 registers with ~200 bytes of spills measured 2 % faster than two blocks at 122)
 template <bool FIELD, int GEOM, bool TRACE>
-__global__ void __launch_bounds__(kBlock, FIELD ? 2 : 4) k_charged(DeviceState D) {
+__global__ void __launch_bounds__(kBlock, FIELD ? 3 : 4) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }
@@ -557,7 +565,7 @@ template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_discrete(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
-  const uint32_t finished_ = ctl->finished;
+  const uint32_t finished_ = ctl->finished | (uint32_t)ctl->error;
   const uint32_t b_an = ctl->rb[R_ANNIH][0], e_an = ctl->re[R_ANNIH][0];
   const uint32_t b_pe = ctl->rb[R_PE][0], e_pe = ctl->re[R_PE][0];
   const uint32_t b_pa = ctl->rb[R_PAIR][0], e_pa = ctl->re[R_PAIR][0];
@@ -593,7 +601,7 @@ template <bool TRACE>
 __global__ void __launch_bounds__(kBlock) k_discrete_masked(DeviceState D) {
   pdl_prologue();
   const Control* ctl = D.ctl;
-  const uint32_t finished_ = ctl->finished;
+  const uint32_t finished_ = ctl->finished | (uint32_t)ctl->error;
   const uint32_t re = D.N;   // (modes none / partition only: every slot, masked by the key byte)
   const uint32_t k_iter = ctl->iter;
   if (finished_) return;

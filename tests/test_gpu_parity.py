@@ -412,3 +412,38 @@ def test_torch_stream_and_workspace(binding):
     ctx.transport(w.primaries, w.n_events)
     assert np.array_equal(ctx.tallies_fixed(), ref["fixed"])
     ctx.close()
+
+
+def test_error_codes(binding):
+    """the sticky device-side errors of include/cel.h are raised, not silently absorbed"""
+    import torch
+    w = W.config1(n_events=4, n_slots=256)
+    # max_steps_per_track outside 1..65535 is rejected at creation (the step count is a 16-bit field)
+    for bad in (0, 70000):
+        w2 = W.config1(n_events=4, n_slots=256); w2.physics["max_steps_per_track"] = bad
+        with pytest.raises(binding.CelError) as ei:
+            binding.from_workload(w2)
+        assert ei.value.code == -1
+    # device-resident primaries are checked as they are loaded: NaN energy -> NONFINITE, bad direction -> INVALID_ARG
+    for field, value, code in (("energy", np.nan, -6), ("energy", np.inf, -6), ("dir", (0.0, 0.0, 2.0), -1), ("pos", (80.0, 0.0, 0.5), -1), ("event", 9, -1)):
+        p = w.primaries.copy(); p[field][1] = value
+        d = torch.from_numpy(p.view(np.uint8).copy()).cuda()
+        ctx = binding.from_workload(w)
+        with pytest.raises(binding.CelError) as ei:
+            ctx.transport_device(d.data_ptr(), len(p), w.n_events)
+            ctx.tallies_view()
+        assert ei.value.code == code, (field, ei.value.code)
+        ctx.close()
+    # a single deposit of 2^63 quanta or more: TALLY_OVERFLOW (1e10 MeV photons: 6.9e20 quanta each)
+    w3 = W.config1(n_events=4, n_slots=256, energy=1e10)
+    ctx = binding.from_workload(w3)
+    with pytest.raises(binding.CelError) as ei:
+        ctx.transport(w3.primaries, w3.n_events)
+        ctx.tallies_view()
+    assert ei.value.code == -5
+    ctx.close()
+    # more than 2^24 events do not fit the slot state's event field
+    ctx = binding.from_workload(w)
+    with pytest.raises(binding.CelError):
+        ctx.transport(w.primaries, (1 << 24) + 1)
+    ctx.close()

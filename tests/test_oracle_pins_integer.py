@@ -336,3 +336,18 @@ def test_reuse_mode_conserves_energy_and_is_sort_consistent():
     c4, c1 = o.counters(), o1.counters()
     assert c4["secondaries"] < 0.8 * c1["secondaries"]
     assert abs(c4["track_steps"] - c1["track_steps"]) < 0.1 * c1["track_steps"]
+
+
+def test_openmp_threads_do_not_change_results():
+    """the oracle's per-slot phases on several host threads (bench.py's all-cores cpu_baseline leg) give bit-identical
+    tallies, counts and counters: slots are independent and the PRNG is counter-based"""
+    import os
+    w = W.config3(n_events=6, n_slots=1 << 12, energy=800.0, seed=77)
+    res = []
+    for n in (1, max(2, min(8, os.cpu_count() or 2))):
+        o = make_oracle(w)
+        o.set_threads(n)
+        o.transport(w.primaries, w.n_events)
+        res.append((o.tallies_fixed(), o.counts(), o.counters(), o.state()))
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1]) and res[0][2] == res[1][2]
+    assert np.array_equal(res[0][3], res[1][3])
