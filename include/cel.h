@@ -138,6 +138,7 @@ enum { CEL_K_FILL_SORT = 0, CEL_K_ANNIH, CEL_K_PE, CEL_K_PAIR, CEL_K_PHOTON, CEL
        CEL_K_PART_COUNT, CEL_K_PART_SCATTER /* the two passes of the charged / neutral partition (CEL_SORT_PARTITION) */,
        CEL_K_DISCRETE /* photoelectric + pair + annihilation in one launch (sort by action, option merge_discrete) */,
        CEL_K_HITS_FLUSH /* option hits = 1: the iteration's hit records streamed to the pinned host ring buffer */,
+       CEL_K_TAIL /* small populations: one block runs whole iterations back to back (option tail) */,
        CEL_KERNEL_COUNT };
 int cel_kernel_count(void);                 /* CEL_KERNEL_COUNT */
 const char* cel_kernel_name(int kernel_id); /* static string, "" if out of range */
@@ -155,6 +156,11 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * branches of the iteration graph; 0 = one after the other. pdl: programmatic dependent launch along the main
  * chain (default 1). merge_discrete: photoelectric + pair + annihilation in one launch (default 1: sorted by action
  * over their three ranges, unsorted / partition as one masked pass before the move kernels; 0: one launch per action).
+ * tail: 1 (default) = when the lagged status shows that live tracks + initializers fit one block (<= 512), the host enqueues
+ * one single-block kernel that runs up to 256 whole iterations back to back instead of batches of the iteration graph, and
+ * switches back if the population grows (the fixed cost of an iteration is exposed at low track counts);
+ * results are bit-identical; not used with hits, trace, profile or CEL_SORT_PARTITION. grid_cap: blocks per SM of the action
+ * kernels' grids (default 8; several contexts sharing the GPU may take a share each).
  * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
  * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);

@@ -4,6 +4,7 @@
 #include "../../include/cel.h"
 #include "cel_kernels.cuh"
 #include "cel_physics.cuh"
+#include "cel_tail.cuh"
 
 #include <cmath>
 #include <condition_variable>
@@ -58,6 +59,8 @@ struct cel_ctx {
   cudaStream_t side[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // branches of the iteration graph (independent action kernels)
   cudaEvent_t ev_fork = nullptr, ev_join[kSideStreams] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   int concurrent = 1;
+  int tail = 1; int tail_iters = 256; int tail_enter = 512;   // k_tail: small populations (cel_tail.cuh)
+  uint64_t tail_launches = 0;
   int grid_cap = 8;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
@@ -485,6 +488,9 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "merge_discrete")) c->merge_discrete = v ? 1 : 0;
   else if (!std::strcmp(name, "trace_ends")) c->trace_ends = v ? 1 : 0;
   else if (!std::strcmp(name, "trace")) { if (v < 0 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->trace_iters = (int)v; }
+  else if (!std::strcmp(name, "tail")) c->tail = v ? 1 : 0;
+  else if (!std::strcmp(name, "tail_iters")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->tail_iters = (int)v; }
+  else if (!std::strcmp(name, "tail_enter")) { if (v < 0 || v > kTailCap) return CEL_ERR_INVALID_ARG; c->tail_enter = (int)v; }
   else if (!std::strcmp(name, "grid_cap")) { if (v < 1 || v > 32) return CEL_ERR_INVALID_ARG; c->grid_cap = (int)v; }
   else if (!std::strcmp(name, "hits")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->hits_mode = (int)v; }
   else if (!std::strcmp(name, "hit_tally")) c->hit_tally = v ? 1 : 0;
@@ -523,7 +529,7 @@ int physics_grid(const cel_ctx* c) {
 
 const char* const kKernelNames[CEL_KERNEL_COUNT] = {
     "fill_sort", "annihilation", "photoelectric", "pair", "photon", "charged", "push",
-    "part_count", "part_scatter", "discrete", "hits_flush"};
+    "part_count", "part_scatter", "discrete", "hits_flush", "tail"};
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
@@ -801,6 +807,16 @@ int load_primaries_host(cel_ctx* c, const cel_primary* p, uint64_t n) {
   return CEL_OK;
 }
 
+// small populations: one single-block kernel runs up to tail_iters whole iterations (cel_tail.cuh)
+void launch_tail(cel_ctx* c) {
+  const bool cyl = c->D.P.geom_kind == CEL_GEOM_CYL, field = c->D.P.bmag != 0.0;
+  const uint32_t n = (uint32_t)c->tail_iters;
+  cudaStream_t s = c->stream;
+  if (cyl) { if (field) k_tail<true, 1><<<1, kTailThreads, 0, s>>>(c->D, n); else k_tail<false, 1><<<1, kTailThreads, 0, s>>>(c->D, n); }
+  else { if (field) k_tail<true, 0><<<1, kTailThreads, 0, s>>>(c->D, n); else k_tail<false, 0><<<1, kTailThreads, 0, s>>>(c->D, n); }
+  c->launches += 1; c->tail_launches += 1;
+}
+
 // enqueue batches of iterations; after each batch copy the control block to pinned memory asynchronously and look
 // at the PREVIOUS batch's copy, so the device always has a batch queued while the host decides
 int run_loop(cel_ctx* c) {
@@ -810,8 +826,27 @@ int run_loop(cel_ctx* c) {
   int slot = 0;
   bool have_prev = false;
   int rc = CEL_OK;
+  // the single-block form for small populations (option tail): chosen batch by batch from the lagged status
+  const bool tail_ok = c->tail && !c->profile && c->hits_mode == 0 && c->trace_iters == 0 && c->D.sort_mode != CEL_SORT_PARTITION;
+  bool in_tail = false;
+  c->tail_launches = 0;
   while (true) {
     int per_iter = c->kernels_per_iteration;
+    if (in_tail) {
+      launch_tail(c);
+      enqueued += c->tail_iters;
+      CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
+      CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
+      const int prev = slot ^ 1;
+      CEL_CUDA(c, cudaEventSynchronize(c->ev_batch[prev]));
+      const Control& st = c->h_status[prev];
+      if (st.error != 0) { rc = st.error; break; }
+      if (st.finished) break;
+      in_tail = (uint64_t)st.alive + st.n_init <= (uint64_t)c->tail_enter;
+      if (enqueued >= c->max_iterations) { rc = CEL_ERR_MAX_ITER; break; }
+      slot ^= 1;
+      continue;
+    }
     // hits, mode 1: the batch about to be enqueued streams into the ring buffer the consumer read two batches ago
     if (c->hits_mode == 1) consumer_wait_idle(c);
     if (c->graph_exec && c->use_graph && !c->profile && c->hits_mode != 2) {
@@ -852,6 +887,7 @@ int run_loop(cel_ctx* c) {
       if (c->hits_mode == 1 && st.hits_in_batch) consumer_submit(c, c->h_ring[st.hits_buf & 1u], st.hits_in_batch);
       if (st.error != 0) { rc = st.error; break; }
       if (st.finished) break;
+      in_tail = tail_ok && st.iterations > 0 && (uint64_t)st.alive + st.n_init <= (uint64_t)c->tail_enter;
     }
     if (enqueued >= c->max_iterations) { rc = CEL_ERR_MAX_ITER; break; }
     have_prev = true;

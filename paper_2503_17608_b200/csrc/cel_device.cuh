@@ -144,6 +144,7 @@ struct DeviceState {
   int sort_mode;          // 0 none, 1 by action, 2 by particle, 3 partition (CEL_SORT_BY_ACTION_REUSE is 1 here, with reuse = 1)
   int reuse;              // S9-R: a slot vacated by its interaction takes its first secondary in place
   int write_vacant;       // 1 = also write the indices of vacant slots (complete permutation, debug surface)
+  int vac_buf_override;   // 0: vacancies created in iteration k go to the counters of parity (k&1)^1; 1 + p: to parity p (k_tail)
   unsigned long long init_capacity;
   uint32_t n_events;
   uint32_t log_capacity;
@@ -178,7 +179,7 @@ struct DeviceState {
 };
 
 // kernel ids of the timeline and of cel_kernel_times (= CEL_K_* of include/cel.h, checked in cel_api.cu)
-enum KernelId : int { K_FILL_SORT = 0, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_HITS_FLUSH, K_COUNT };
+enum KernelId : int { K_FILL_SORT = 0, K_ANNIH, K_PE, K_PAIR, K_PHOTON, K_CHARGED, K_PUSH, K_PART_COUNT, K_PART_SCATTER, K_DISCRETE, K_HITS_FLUSH, K_TAIL, K_COUNT };
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;

@@ -150,7 +150,7 @@ __device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, uint
     warp_aggregated_add32(D.tile_sec, tile, (uint32_t)nsec);
   }
   if (action == A_VACANT) {   // into the buffer the fill of iteration k+1 reads (parity (k+1)&1)
-    const uint32_t q = (k_iter & 1u) ^ 1u;
+    const uint32_t q = D.vac_buf_override ? (uint32_t)(D.vac_buf_override - 1) : (k_iter & 1u) ^ 1u;
     warp_aggregated_add32(D.tile_vac + (size_t)q * D.n_tiles, tile, 1u);
   }
 }

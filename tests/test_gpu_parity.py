@@ -447,3 +447,20 @@ def test_error_codes(binding):
     with pytest.raises(binding.CelError):
         ctx.transport(w.primaries, (1 << 24) + 1)
     ctx.close()
+
+
+@pytest.mark.parametrize("mode", [1, 0, 2, 4])
+def test_tail_kernel_identical(binding, mode):
+    """small populations run in one single-block kernel, many iterations per launch (cel_tail.cuh, option tail, the
+    default): tallies, per-iteration counts and counters are bit-identical to the kernel-per-phase form, also when the
+    two forms alternate every few iterations (tail_iters = 3: every exit leaves the bookkeeping of the other form intact)"""
+    for w0 in (W.config3(n_events=6, n_slots=1 << 13, energy=400.0), W.config4(n_events=2, per_event=4, n_slots=1 << 13),
+               W.config2(n_events=3, n_slots=5000, energy=150.0)):
+        w0.sort_mode = mode
+        ref, cref = run_gpu(binding, w0, tail=0)
+        for opts in (dict(tail=1), dict(tail=1, tail_iters=3, batch=2), dict(tail=1, tail_enter=64, batch=4), dict(tail=1, use_graph=0, batch=3, tail_iters=7)):
+            a, ca = run_gpu(binding, w0, **opts)
+            assert np.array_equal(a["fixed"], ref["fixed"]) and np.array_equal(ca, cref), (w0.name, mode, opts)
+            assert a["track_steps"] == ref["track_steps"] and a["secondaries"] == ref["secondaries"] and a["iterations"] == ref["iterations"]
+        a, _ = run_gpu(binding, w0, tail=1)
+        assert a["kernel_launches"] < ref["kernel_launches"]          # the tail form was used
