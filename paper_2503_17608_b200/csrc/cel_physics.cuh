@@ -380,113 +380,147 @@ __global__ void __launch_bounds__(kBlock, 4) k_photon(DeviceState D) {
 }
 
 // ================================================================ charged: bremsstrahlung (S8) then move (S7)
-// S7: step limit -> linear or helical propagation (<= max_substeps chord substeps) -> CSDA loss -> MSC -> fate
-template <bool FIELD, int GEOM>
-__device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, double& eesc) {
+// S7: step limit -> linear or helical propagation (<= max_substeps chord substeps) -> CSDA loss -> MSC -> fate.
+// The move is written in three parts: step limit (charged_limit), propagation (one straight segment, or chord substeps
+// of the helix one at a time), and energy loss + MSC + fate (charged_finish).
+struct ChargedStep {      // what the step limit leaves for the parts after the propagation
+  double T0, p2, r0, s_phys;
+  int mat, j0, vol0;
+  bool interaction_wins;
+};
+struct Prop {             // propagation state of one track in a field (S7.3), advanced one chord substep at a time
+  double x, y, z, dx, dy, dz, remaining, travelled, omega, h_max;
+  int vol, surf, n;
+  int escaped, complete;
+};
+
+// S7.1 + S7.2. Returns false if the track stopped at once (S7.1; `action` is then its fate), true if it moves.
+__device__ __forceinline__ bool charged_limit(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, ChargedStep& c, int& action) {
   const Params& P = D.P;
-  const int vol0 = t.vol;
-  const int ptype = t.ptype;
+  c.vol0 = t.vol;
   if (t.nsteps < 65535u) t.nsteps += 1;
-  const double T0 = t.a.energy;
-  if (T0 < P.cut) {  // S7.1
-    edep += T0;
+  c.T0 = t.a.energy;
+  if (c.T0 < P.cut) {  // S7.1
+    edep += c.T0;
     t.a.energy = 0.0;
-    return stop_charged(P, ptype, edep);
+    action = stop_charged(P, t.ptype, edep);
+    return false;
   }
-  const int mat = __ldg(P.vol_material + t.vol);
-  const double p2 = T0 * (T0 + 2.0 * kElectronMass);   // p^2; beta p = p^2 / (T0 + m_e)
+  c.mat = __ldg(P.vol_material + t.vol);
+  c.p2 = c.T0 * (c.T0 + 2.0 * kElectronMass);   // p^2; beta p = p^2 / (T0 + m_e)
   // S7.2 step limit
-  double r0 = 0.0, s_r = CEL_INF, s_d = CEL_INF;
-  int j0 = 0;
-  if (mat >= 0) {
-    const GridPos g = grid_locate(P, T0);
-    j0 = g.j;
-    const double2* cxs = reinterpret_cast<const double2*>(P.charged_xs + (size_t)mat * kGrid + g.j);  // nodes j, j+1
+  c.r0 = 0.0; c.j0 = 0;
+  double s_r = CEL_INF, s_d = CEL_INF;
+  if (c.mat >= 0) {
+    const GridPos g = grid_locate(P, c.T0);
+    c.j0 = g.j;
+    const double2* cxs = reinterpret_cast<const double2*>(P.charged_xs + (size_t)c.mat * kGrid + g.j);  // nodes j, j+1
     const double2 n0 = __ldg(cxs);
     const double2 n1 = __ldg(cxs + 1);
     if (P.enable_eloss) {
-      r0 = lerp_node(n0.y, n1.y, g.f);
-      s_r = (r0 <= kRhoF) ? r0 : fmax(kAlphaR * r0, kRhoF);
+      c.r0 = lerp_node(n0.y, n1.y, g.f);
+      s_r = (c.r0 <= kRhoF) ? c.r0 : fmax(kAlphaR * c.r0, kRhoF);
     }
     const double sb = lerp_node(n0.x, n1.x, g.f);
     double xi0, xi1;
     draw_pair(P, slot, k_iter, PH_STEP, 0, xi0, xi1);
     if (sb > 0.0) s_d = -log(xi0) / sb;
   }
-  const bool interaction_wins = s_d < s_r;
-  const double s_phys = interaction_wins ? s_d : s_r;
-  // S7.3 propagation
-  double travelled = 0.0;
-  bool escaped = false, complete = false;
-  if (!FIELD) {
-    int which;
-    const double s_b = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, s_phys, which);
-    if (s_phys < s_b) {
-      t.a.x += s_phys * t.dx; t.a.y += s_phys * t.dy; t.a.z += s_phys * t.dz;
-      t.surf = -1; travelled = s_phys; complete = true;
-    } else {
-      t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
-      travelled = s_b;
-      escaped = cross_boundary<GEOM>(P, t.a.z, t.dz, t.vol, t.surf, which);
-    }
+  c.interaction_wins = s_d < s_r;
+  c.s_phys = c.interaction_wins ? s_d : s_r;
+  return true;
+}
+
+// S7.3 without a field: one straight segment
+template <int GEOM>
+__device__ __forceinline__ void propagate_linear(const Params& P, Track& t, double s_phys, double& travelled, bool& escaped, bool& complete) {
+  int which;
+  const double s_b = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, t.dx, t.dy, t.dz, t.vol, t.surf, s_phys, which);
+  if (s_phys < s_b) {
+    t.a.x += s_phys * t.dx; t.a.y += s_phys * t.dy; t.a.z += s_phys * t.dz;
+    t.surf = -1; travelled = s_phys; complete = true;
   } else {
-    const double q = (ptype == P_ELECTRON) ? -1.0 : 1.0;
-    const double omega = q * kKappa * P.bmag / sqrt(p2);
-    const double h_max = fmin(sqrt(8.0 * kDeltaChord / fabs(omega)), 0.5 / fabs(omega));
-    double remaining = s_phys;
-    int n = 0;
-    if (!(s_phys > 0.0)) complete = true;
-    while (!complete) {
-      if (n == P.max_substeps) break;  // paused: the remainder is re-sampled next iteration
-      double h = fmin(remaining, h_max);
-      const HelixFrame F = helix_frame(P, t.dx, t.dy, t.dz);
-      // The chord c = pos(h) - pos is used UN-normalised: the distance to the boundary along it then comes out in units of
-      // the chord (f = t / |c| of S7.3 directly), "t <= |c|" is "f <= 1", and the sign tests of the dip rule and of the
-      // crossing do not care about the scale — no square root and no three divisions per substep (the same reals as S7.3,
-      // rounded differently in the last place)
-      double nx, ny, nz, ndx, ndy, ndz, cx, cy, cz, fb;
-      int which;
-      for (int halvings = 0;; ++halvings) {
-        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, h, nx, ny, nz, ndx, ndy, ndz);
-        cx = nx - t.a.x; cy = ny - t.a.y; cz = nz - t.a.z;
-        fb = distance_to_boundary<GEOM>(P, t.a.x, t.a.y, t.a.z, cx, cy, cz, t.vol, t.surf, 1.0, which);
-        // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
-        if (fb == 0.0 && halvings < kMaxDipHalvings &&
-            tangent_points_inward(P, t.a.x, t.a.y, t.dx, t.dy, t.dz, cx, cy, cz, which)) { h *= 0.5; continue; }
-        break;
-      }
-      if (fb <= 1.0) {
-        double fx, fy, fz, fdx, fdy, fdz;
-        helix_point(P, F, t.a.x, t.a.y, t.a.z, omega, fb * h, fx, fy, fz, fdx, fdy, fdz);
-        t.a.x += fb * cx; t.a.y += fb * cy; t.a.z += fb * cz;
-        normalise3(fdx, fdy, fdz);
-        t.dx = fdx; t.dy = fdy; t.dz = fdz;
-        travelled += fb * h;
-        escaped = cross_boundary<GEOM>(P, t.a.z, cz, t.vol, t.surf, which);
-        break;
-      }
-      normalise3(ndx, ndy, ndz);
-      t.a.x = nx; t.a.y = ny; t.a.z = nz;
-      t.dx = ndx; t.dy = ndy; t.dz = ndz;
-      travelled += h;
-      t.surf = -1;
-      remaining -= h;
-      n += 1;
-      if (remaining <= 0.0) { travelled = s_phys; complete = true; }
-    }
+    t.a.x += s_b * t.dx; t.a.y += s_b * t.dy; t.a.z += s_b * t.dz;
+    travelled = s_b;
+    escaped = cross_boundary<GEOM>(P, t.a.z, t.dz, t.vol, t.surf, which);
   }
+}
+
+// S7.3 in a field: set up the chord substeps. Returns false if there is nothing to propagate (s_phys = 0).
+__device__ __forceinline__ bool prop_begin(const Params& P, const Track& t, const ChargedStep& c, Prop& s) {
+  s.x = t.a.x; s.y = t.a.y; s.z = t.a.z; s.dx = t.dx; s.dy = t.dy; s.dz = t.dz;
+  s.vol = t.vol; s.surf = t.surf; s.n = 0; s.escaped = 0; s.complete = 0;
+  s.travelled = 0.0; s.remaining = c.s_phys;
+  const double q = (t.ptype == P_ELECTRON) ? -1.0 : 1.0;
+  s.omega = q * kKappa * P.bmag / sqrt(c.p2);
+  s.h_max = fmin(sqrt(8.0 * kDeltaChord / fabs(s.omega)), 0.5 / fabs(s.omega));
+  if (!(c.s_phys > 0.0)) { s.complete = 1; return false; }
+  return true;
+}
+// one chord substep (S7.3). Returns true while another substep is due in this iteration (not complete, no boundary met,
+// fewer than max_substeps made: otherwise the step is paused, and the remainder re-sampled next iteration).
+template <int GEOM>
+__device__ __forceinline__ bool helix_substep(const Params& P, Prop& s) {
+  double h = fmin(s.remaining, s.h_max);
+  const HelixFrame F = helix_frame(P, s.dx, s.dy, s.dz);
+  // The chord c = pos(h) - pos is used UN-normalised: the distance to the boundary along it then comes out in units of
+  // the chord (f = t / |c| of S7.3 directly), "t <= |c|" is "f <= 1", and the sign tests of the dip rule and of the
+  // crossing do not care about the scale — no square root and no three divisions per substep (the same reals as S7.3,
+  // rounded differently in the last place)
+  double nx, ny, nz, ndx, ndy, ndz, cx, cy, cz, fb;
+  int which;
+  for (int halvings = 0;; ++halvings) {
+    helix_point(P, F, s.x, s.y, s.z, s.omega, h, nx, ny, nz, ndx, ndy, ndz);
+    cx = nx - s.x; cy = ny - s.y; cz = nz - s.z;
+    fb = distance_to_boundary<GEOM>(P, s.x, s.y, s.z, cx, cy, cz, s.vol, s.surf, 1.0, which);
+    // S7.3 dip rule: on a surface with the tangent into the volume but the chord out of it, halve h
+    if (fb == 0.0 && halvings < kMaxDipHalvings &&
+        tangent_points_inward(P, s.x, s.y, s.dx, s.dy, s.dz, cx, cy, cz, which)) { h *= 0.5; continue; }
+    break;
+  }
+  if (fb <= 1.0) {
+    double fx, fy, fz, fdx, fdy, fdz;
+    helix_point(P, F, s.x, s.y, s.z, s.omega, fb * h, fx, fy, fz, fdx, fdy, fdz);
+    s.x += fb * cx; s.y += fb * cy; s.z += fb * cz;
+    normalise3(fdx, fdy, fdz);
+    s.dx = fdx; s.dy = fdy; s.dz = fdz;
+    s.travelled += fb * h;
+    s.escaped = cross_boundary<GEOM>(P, s.z, cz, s.vol, s.surf, which) ? 1 : 0;
+    return false;
+  }
+  normalise3(ndx, ndy, ndz);
+  s.x = nx; s.y = ny; s.z = nz;
+  s.dx = ndx; s.dy = ndy; s.dz = ndz;
+  s.travelled += h;
+  s.surf = -1;
+  s.remaining -= h;
+  s.n += 1;
+  if (s.remaining <= 0.0) { s.complete = 1; return false; }
+  return s.n < P.max_substeps;
+}
+__device__ __forceinline__ void prop_end(const Prop& s, const ChargedStep& c, Track& t, double& travelled, bool& escaped, bool& complete) {
+  t.a.x = s.x; t.a.y = s.y; t.a.z = s.z; t.dx = s.dx; t.dy = s.dy; t.dz = s.dz; t.vol = s.vol; t.surf = s.surf;
+  escaped = s.escaped != 0; complete = s.complete != 0;
+  travelled = complete ? c.s_phys : s.travelled;
+}
+
+// S7.4 - S7.6: energy loss over the travelled path, multiple scattering, fate. Returns the next action.
+__device__ __forceinline__ int charged_finish(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, const ChargedStep& c,
+                                              double travelled, bool escaped, bool complete, double& edep, double& eesc) {
+  const Params& P = D.P;
+  const int ptype = t.ptype;
   // S7.4 energy loss
-  double T1 = T0;
-  if (mat >= 0 && P.enable_eloss) {
-    const double r1 = r0 - travelled;
-    T1 = (r1 <= 0.0) ? 0.0 : range_inverse(P, P.range_tab + (size_t)mat * kGrid, r1, j0);
-    if (T1 > T0) T1 = T0;
-    edep += T0 - T1;
+  double T1 = c.T0;
+  if (c.mat >= 0 && P.enable_eloss) {
+    const double r1 = c.r0 - travelled;
+    T1 = (r1 <= 0.0) ? 0.0 : range_inverse(P, P.range_tab + (size_t)c.mat * kGrid, r1, c.j0);
+    if (T1 > c.T0) T1 = c.T0;
+    edep += c.T0 - T1;
   }
   // S7.5 multiple scattering
-  if (P.enable_msc && !escaped && mat >= 0 && travelled > 0.0 && T1 >= P.cut) {
-    const double x = travelled * __ldg(&P.mats[mat].inv_X0);
-    const double theta0 = 13.6 * (T0 + kElectronMass) / p2 * sqrt(x) * fmax(0.0, 1.0 + 0.038 * log(x));
+  if (P.enable_msc && !escaped && c.mat >= 0 && travelled > 0.0 && T1 >= P.cut) {
+    const double x = travelled * __ldg(&P.mats[c.mat].inv_X0);
+    const double theta0 = 13.6 * (c.T0 + kElectronMass) / c.p2 * sqrt(x) * fmax(0.0, 1.0 + 0.038 * log(x));
     double xm0, xm1;
     draw_pair(P, slot, k_iter, PH_MSC, 0, xm0, xm1);
     const double theta = fmin(theta0 * sqrt(-2.0 * log(xm0)), kPi);
@@ -498,7 +532,7 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
   const double rest = (ptype == P_POSITRON) ? 2.0 * kElectronMass : 0.0;
   if (escaped) {
     eesc += T1 + rest; t.a.energy = T1;
-    if (t.vol < 0 || t.vol > 254) t.vol = vol0;
+    if (t.vol < 0 || t.vol > 254) t.vol = c.vol0;
     return A_VACANT;
   }
   if (T1 < P.cut) {
@@ -510,7 +544,27 @@ __device__ __forceinline__ int move_charged(const DeviceState& D, uint32_t slot,
     return A_VACANT;
   }
   t.a.energy = T1;
-  return (interaction_wins && complete) ? A_BREMS : A_MOVE_C;
+  return (c.interaction_wins && complete) ? A_BREMS : A_MOVE_C;
+}
+
+// S8 bremsstrahlung (act = BREMS): k log-uniform on [k_c, T], photon collinear. Returns the action after it: MOVE_C (the
+// track goes on and moves in this iteration), or its fate if it stopped.
+__device__ __forceinline__ int brems(const DeviceState& D, uint32_t slot, uint32_t k_iter, Track& t, double& edep, int& nsec) {
+  const Params& P = D.P;
+  double xi0, xi1;
+  draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
+  const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
+  const double T1 = t.a.energy - kph;
+  if (T1 < P.cut) {
+    edep += T1;
+    int action = stop_charged(P, t.ptype, edep);
+    if (D.reuse && action == A_VACANT) action = become_secondary(t, kph, t.dx, t.dy, t.dz, P_GAMMA);   // S9-R: the photon takes the slot
+    else { stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA); t.a.energy = 0.0; }
+    return action;
+  }
+  stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
+  t.a.energy = T1;
+  return A_MOVE_C;
 }
 
 // act = BREMS: interact, then (unless the track stopped) move; act = MOVE_C: move
@@ -522,26 +576,31 @@ __device__ __forceinline__ void do_charged(const DeviceState& D, uint32_t slot, 
   double edep = 0.0, eesc = 0.0;
   int nsec = 0;
   int action = A_MOVE_C;
-  if (act == A_BREMS) {  // S8: k log-uniform on [k_c, T]; photon collinear
-    double xi0, xi1;
-    draw_pair(P, slot, k_iter, PH_INTERACT, 0, xi0, xi1);
-    const double kph = P.cut * exp(xi0 * log(t.a.energy / P.cut));
-    const double T1 = t.a.energy - kph;
-    if (T1 < P.cut) {
-      edep += T1;
-      action = stop_charged(P, t.ptype, edep);
-      if (D.reuse && action == A_VACANT) action = become_secondary(t, kph, t.dx, t.dy, t.dz, P_GAMMA);   // S9-R: the photon takes the slot
-      else { stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA); t.a.energy = 0.0; }
-    } else {
-      stage_secondary(D, slot, nsec++, t, kph, t.dx, t.dy, t.dz, P_GAMMA);
-      t.a.energy = T1;
+  if (act == A_BREMS) action = brems(D, slot, k_iter, t, edep, nsec);
+  if (action == A_MOVE_C) {
+    ChargedStep c;
+    if (charged_limit(D, slot, k_iter, t, edep, c, action)) {
+      double travelled = 0.0;
+      bool escaped = false, complete = false;
+      if (!FIELD) {
+        propagate_linear<GEOM>(P, t, c.s_phys, travelled, escaped, complete);
+      } else {
+        Prop s;
+        if (prop_begin(P, t, c, s)) while (helix_substep<GEOM>(P, s)) {}
+        prop_end(s, c, t, travelled, escaped, complete);
+      }
+      action = charged_finish(D, slot, k_iter, t, c, travelled, escaped, complete, edep, eesc);
     }
   }
-  if (action == A_MOVE_C) action = move_charged<FIELD, GEOM>(D, slot, k_iter, t, edep, eesc);
   finish(D, slot, k_iter, t, action, vol0, edep, eesc, nsec, true);
 }
 // (without a field: four blocks per SM = 64 registers, the count the kernel is tuned at — 70+ registers measured 19 % slower;
-// with a field: three blocks per SM = 85 registers with ~200 bytes of spills measured 2 % faster than two blocks at 122)
+// with a field: three blocks per SM = 85 registers with ~200 bytes of spills measured 2 % faster than two blocks at 122.
+// Tried and dropped for the field kernel: the block parks its tracks' propagation state in shared memory and makes the chord
+// substeps in rounds over a compacted queue, so that warps stay full whatever the mix of 1-substep and 10-substep tracks
+// (12.7 of 32 lanes are active inside the per-thread loop): bit-identical, 40 % fewer warp instructions in the loop, but
+// 22 % SLOWER on config 3 (20.7 vs 16.9 ms) — every warp of the block then waits at the round barriers for the block's
+// slowest track, and the kernel is bound by latency, not by issue slots. DESIGN.md section 10.)
 template <bool FIELD, int GEOM, bool TRACE>
 __global__ void __launch_bounds__(kBlock, FIELD ? 3 : 4) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
