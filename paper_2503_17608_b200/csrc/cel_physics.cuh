@@ -182,6 +182,21 @@ __device__ __forceinline__ Track unpack(const RecA& a, const RecB& b) {
   for (uint32_t i_ = blockIdx.x * blockDim.x + threadIdx.x, tid = i_ < n0_ ? rb0_ + i_ : rb1_ + (i_ - n0_); i_ < n_; \
        i_ += gridDim.x * blockDim.x, tid = i_ < n0_ ? rb0_ + i_ : rb1_ + (i_ - n0_))
 
+// Sorted by action a thread walks its kernel's ranges with a grid stride: the slot of its NEXT index is read together with
+// the current one, and that slot's two records are prefetched into L1 once the current records have arrived, so that the
+// index -> record round trips of all but a thread's first track overlap the arithmetic of the track before.
+#define CEL_NEXT_SLOT()                                                                                      \
+  uint32_t next_slot_ = 0xffffffffu;                                                                         \
+  if (D.sort_mode == 1) {                                                                                    \
+    const uint32_t in_ = i_ + gridDim.x * blockDim.x;                                                        \
+    if (in_ < n_) next_slot_ = D.indices[in_ < n0_ ? rb0_ + in_ : rb1_ + (in_ - n0_)];                        \
+  }
+#define CEL_PREFETCH_NEXT()                                                                                  \
+  if (next_slot_ != 0xffffffffu) {                                                                           \
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(D.stB + next_slot_));                                      \
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(D.stA + next_slot_));                                      \
+  }
+
 __device__ __forceinline__ uint32_t slot_of(const DeviceState& D, uint32_t tid) { return (D.sort_mode == 1 || D.sort_mode == 2) ? D.indices[tid] : tid; }
 
 // S8 photoelectric: the photon's energy goes to an electron along d (or is deposited when electrons are local)
@@ -370,10 +385,12 @@ template <int GEOM, bool TRACE>
 __global__ void __launch_bounds__(kBlock, 4) k_photon(DeviceState D) {
   CEL_FOR_RANGE(R_PHOTON, K_PHOTON) {
     const uint32_t slot = slot_of(D, tid);
+    CEL_NEXT_SLOT()
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_COMPTON && ak != A_MOVE_G) continue; }
     const RecB b = load_b(D.stB + slot);
     const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     const int act = meta_action(b.meta);
+    CEL_PREFETCH_NEXT()
     if (act != A_COMPTON && act != A_MOVE_G) continue;
     do_photon<GEOM>(D, slot, k_iter, a, b, act);
   }
@@ -605,10 +622,12 @@ template <bool FIELD, int GEOM, bool TRACE>
 __global__ void __launch_bounds__(kBlock, FIELD ? 3 : 4) k_charged(DeviceState D) {
   CEL_FOR_RANGE(R_CHARGED, K_CHARGED) {
     const uint32_t slot = slot_of(D, tid);
+    CEL_NEXT_SLOT()
     if (D.sort_mode != 1) { const int ak = D.akey[slot] & 0xf; if (ak != A_MOVE_C && ak != A_BREMS) continue; }
     const RecB b = load_b(D.stB + slot);
     const RecA a = load_a(D.stA + slot);   // issued with b: one round trip, not two
     const int act = meta_action(b.meta);
+    CEL_PREFETCH_NEXT()
     if (act != A_MOVE_C && act != A_BREMS) continue;
     do_charged<FIELD, GEOM>(D, slot, k_iter, a, b, act);
   }
