@@ -160,7 +160,7 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * one single-block kernel that runs up to 256 whole iterations back to back instead of batches of the iteration graph, and
  * switches back if the population grows (the fixed cost of an iteration is exposed at low track counts);
  * results are bit-identical; not used with hits, trace, profile or CEL_SORT_PARTITION. grid_cap: blocks per SM of the action
- * kernels' grids (default 8; several contexts sharing the GPU may take a share each).
+ * kernels' grids (default 6, measured 1 % faster than 8 on config 2; several contexts sharing the GPU may take a share each).
  * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
  * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);

@@ -11,12 +11,19 @@
 // over slots in ascending order, following docs/PHYSICS_SPEC.md S0-S11 in its order and notation.
 // The physics formulas are those the spec freezes from BASELINE.json (north_star, configs).
 //
-// Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers re-derived with Python
-// big integers; Thomson limit and quadrature of the KN differential cross-section; exp(-mu x)
+// Pins (tests/test_oracle_pins_*.py, -m "not gpu"): Philox known answers re-derived with Python
+// big integers; Thomson limit and quadrature of the KN differential cross-section; the textbook
+// non-relativistic and ultra-relativistic limits of the electron stopping power; exp(-mu x)
 // attenuation; KN sampler chi-square and moments vs the analytic pdf; CSDA range vs adaptive
 // quadrature of 1/S; helix radius p/(|q|B) and circle membership; geometry distances vs
-// ray marching; brems/pair/annihilation distribution checks; per-event energy conservation;
-// init/sort/push vs an independent numpy restatement; sort-mode invariance.
+// ray marching; hand-written (vol, surf) crossing sequences in concentric cylinder shells;
+// the tally bin of a step = the volume at the START of the iteration (deposit of a crossing /
+// escaping step computed from the range table in the test); the looper-cap fate (escape credit
+// T, or T + 2 m_e for e+, after exactly max_steps_per_track steps); brems / pair / annihilation /
+// Highland distribution checks; per-event energy conservation; init / sort / push vs an
+// independent numpy restatement; the partition rule (mode 3) and the parent-slot reuse rule
+// (mode 4) hand-worked and restated against mode 1; sort-mode invariance; OpenMP threads do not
+// change a bit.
 // Parity unpinned (no external truth exists): per-layer shower profiles of the simplified
 // physics (configs 2-5) — sanity checks only (shower maximum, containment).
 //

@@ -6,6 +6,17 @@
 #include "cel_physics.cuh"
 #include "cel_tail.cuh"
 
+// NVTX ranges around every enqueued phase (ScopedProfiling over NVTX): compile-time switch, build with
+// -DCEL_NVTX (paper_2503_17608_b200/build.py: CEL_NVTX=1 in the environment); header-only NVTX 3, no library to link
+#ifdef CEL_NVTX
+#include <nvtx3/nvToolsExt.h>
+#define CEL_RANGE_PUSH(name) nvtxRangePushA(name)
+#define CEL_RANGE_POP() nvtxRangePop()
+#else
+#define CEL_RANGE_PUSH(name) ((void)0)
+#define CEL_RANGE_POP() ((void)0)
+#endif
+
 #include <cmath>
 #include <condition_variable>
 #include <cstdio>
@@ -61,7 +72,7 @@ struct cel_ctx {
   int concurrent = 1;
   int tail = 1; int tail_iters = 256; int tail_enter = 512;   // k_tail: small populations (cel_tail.cuh)
   uint64_t tail_launches = 0;
-  int grid_cap = 8;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
+  int grid_cap = 6;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
@@ -533,6 +544,7 @@ const char* const kKernelNames[CEL_KERNEL_COUNT] = {
 
 // bookkeeping after each kernel launch: which kernel it was and, in profile mode, an event behind it
 inline void after_launch(cel_ctx* c, int id, int& n) {
+  CEL_RANGE_PUSH(kKernelNames[id]); CEL_RANGE_POP();   // (a marker-like range per phase: the launch itself is asynchronous)
   c->iter_kernel[n] = id;
   ++n;
   if (c->profile) cudaEventRecord(c->prof_ev[(size_t)c->prof_b * (kMaxKernelsPerIteration + 1) + n], c->stream);
@@ -637,7 +649,12 @@ int enqueue_iteration_t(cel_ctx* c) {
   enqueue_push_and_flush<TR>(c, n);
   return n;
 }
-int enqueue_iteration(cel_ctx* c) { return c->trace_iters > 0 ? enqueue_iteration_t<true>(c) : enqueue_iteration_t<false>(c); }
+int enqueue_iteration(cel_ctx* c) {
+  CEL_RANGE_PUSH("cel:step_iteration");   // P1+P2 fill_sort, P3/P4 action kernels, P5 push (one range per enqueued iteration)
+  const int n = c->trace_iters > 0 ? enqueue_iteration_t<true>(c) : enqueue_iteration_t<false>(c);
+  CEL_RANGE_POP();
+  return n;
+}
 
 // profile mode: add the event-to-event times of the `n_iter` iterations of the batch that just ended
 int collect_profile(cel_ctx* c, int n_iter, int kernels_per_iteration) {
@@ -821,6 +838,8 @@ void launch_tail(cel_ctx* c) {
 // at the PREVIOUS batch's copy, so the device always has a batch queued while the host decides
 int run_loop(cel_ctx* c) {
   cudaStream_t s = c->stream;
+  CEL_RANGE_PUSH("cel:transport_loop");
+  struct RangeGuard { ~RangeGuard() { CEL_RANGE_POP(); } } range_guard;
   CEL_CUDA(c, cudaEventRecord(c->ev_start, s));
   int64_t enqueued = 0;
   int slot = 0;
@@ -833,7 +852,7 @@ int run_loop(cel_ctx* c) {
   while (true) {
     int per_iter = c->kernels_per_iteration;
     if (in_tail) {
-      launch_tail(c);
+      CEL_RANGE_PUSH("cel:tail_batch"); launch_tail(c); CEL_RANGE_POP();
       enqueued += c->tail_iters;
       CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
       CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
