@@ -77,9 +77,9 @@ __device__ __forceinline__ void score(const DeviceState& D, uint32_t event, int 
   }
   const long long q_esc = quantise(eesc);
   if (q_esc != 0) warp_aggregated_add64(D.tally, row + (unsigned long long)D.P.n_bins, (unsigned long long)q_esc);
-  // S10: a single deposit of 2^63 quanta = 2^27 MeV or more (the conversion saturates), a negative or a non-finite
-  // deposit: sticky CEL_ERR_TALLY_OVERFLOW (deposits are never negative in this physics)
-  if (!(edep < 134217728.0) || !(eesc < 134217728.0) || (q_dep | q_esc) < 0) D.ctl->error = -5;
+  // S10: a single deposit of 2^63 quanta = 2^27 MeV or more (the conversion saturates to the largest integer), a negative
+  // or a non-finite one (the most negative integer): sticky CEL_ERR_TALLY_OVERFLOW. q + 1 has its top bit set in all of them.
+  if ((((unsigned long long)q_dep + 1ull) | ((unsigned long long)q_esc + 1ull)) >> 63) D.ctl->error = -5;
   if (D.hits != nullptr) {   // the same integers, as records for the host (a measurement / application mode)
     append_hit(D, q_dep != 0 && bin >= 0, event, bin, (unsigned long long)q_dep);
     append_hit(D, q_esc != 0, event, D.P.n_bins, (unsigned long long)q_esc);
@@ -124,8 +124,9 @@ __device__ __forceinline__ int stop_charged(const Params& P, int ptype, double& 
 __device__ __forceinline__ void finish(const DeviceState& D, uint32_t slot, uint32_t k_iter, const Track& t, int action, int vol0, double edep,
                                        double eesc, int nsec, bool write_a) {
   score(D, t.event, vol0, edep, eesc);
-  // a non-finite energy, position or direction must not go on (grid_locate would send a NaN to cell 0): sticky CEL_ERR_NONFINITE
-  if (!isfinite(((t.a.x + t.a.y) + (t.a.z + t.a.energy)) + ((t.dx + t.dy) + t.dz))) D.ctl->error = -6;
+  // a non-finite energy or position must not go on (grid_locate would send a NaN to cell 0): sticky CEL_ERR_NONFINITE.
+  // Exponent-field tests (a few integer operations; a non-finite direction shows in the position one step later).
+  if ((((__double2hiint(t.a.energy) & 0x7ff00000) == 0x7ff00000) | ((__double2hiint((t.a.x + t.a.y) + t.a.z) & 0x7ff00000) == 0x7ff00000))) D.ctl->error = -6;
   const uint32_t tile = slot >> D.tile_shift;
   if (D.reuse && action == A_VACANT && nsec >= 1) {
     // S9-R, the general case (the interaction epilogues handle theirs without staging): the slot ends the iteration
