@@ -74,6 +74,7 @@ struct cel_ctx {
   uint64_t tail_launches = 0;
   int grid_cap = 6;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
+  bool no_pdl_next = false;
   int pdl = 1;   // programmatic dependent launch along the main-stream chain of an iteration
   cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_batch[kStatusSlots] = {nullptr, nullptr};
   Control* h_status = nullptr;      // pinned, kStatusSlots entries
@@ -558,7 +559,10 @@ void launch_chain(cel_ctx* c, K kernel, int grid, int block, cudaStream_t s) {
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = attr; cfg.numAttrs = (c->pdl && !c->profile) ? 1 : 0;
+  // (the first kernel after a k_tail launch is serialised fully: k_fill_sort reads counters and key bytes BEFORE its
+  // programmatic-dependency wait, which is only sound when the kernel before it wrote none of them)
+  cfg.attrs = attr; cfg.numAttrs = (c->pdl && !c->profile && !c->no_pdl_next) ? 1 : 0;
+  c->no_pdl_next = false;
   cudaLaunchKernelEx(&cfg, kernel, c->D);
 }
 
@@ -832,6 +836,7 @@ void launch_tail(cel_ctx* c) {
   if (cyl) { if (field) k_tail<true, 1><<<1, kTailThreads, 0, s>>>(c->D, n); else k_tail<false, 1><<<1, kTailThreads, 0, s>>>(c->D, n); }
   else { if (field) k_tail<true, 0><<<1, kTailThreads, 0, s>>>(c->D, n); else k_tail<false, 0><<<1, kTailThreads, 0, s>>>(c->D, n); }
   c->launches += 1; c->tail_launches += 1;
+  c->no_pdl_next = true;
 }
 
 // enqueue batches of iterations; after each batch copy the control block to pinned memory asynchronously and look

@@ -171,8 +171,9 @@ __device__ __forceinline__ uint32_t filled_by_plan(uint32_t v, uint32_t prefix, 
   return lo + (end > hs ? end - hs : 0u);
 }
 // returns true if the tile's key bytes were read (false: the tile is entirely vacant and gets no fill)
+// kv0: the key bytes of the thread's four slots in sub-tile 0, loaded by the caller ahead of time
 __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, const FillPlan pl,
-                                          uint32_t prefix, uint32_t tile_vacant) {
+                                          uint32_t prefix, uint32_t tile_vacant, uint32_t kv0) {
   uint32_t rank0 = prefix;                                   // rank of the first vacancy of the current sub-tile
   const uint32_t rank_end = prefix + tile_vacant;            // one past the rank of the tile's last vacancy
   const uint32_t real = real_slots_in_tile(D, tile);
@@ -184,7 +185,7 @@ __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, ui
   for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
     const uint32_t sub_base = (tile << D.tile_shift) + sub * kSub;
     const uint32_t base = sub_base + threadIdx.x * kKeysPerThread;
-    uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + base);
+    uint32_t kv = sub == 0 ? kv0 : *reinterpret_cast<const uint32_t*>(D.akey + base);
     uint32_t* skey = sm.skey + (sub < (uint32_t)kResidentSubs ? sub : 0u) * kTileThreads;   // (beyond kResidentSubs: scratch only)
     uint8_t* skey_b = reinterpret_cast<uint8_t*>(skey);
     if (rank0 < rank_end && filled_by_plan(rank_end - rank0, rank0, pl) != 0) {   // block-uniform: this sub-tile may have vacancies to fill
@@ -269,6 +270,40 @@ constexpr uint32_t kSpinLimit = 1u << 24;   // polls before a wait gives up (~ a
 // The caller sets sm.base[key] and synchronises. Vacant slots are never launched: their indices are written only when
 // the complete permutation is asked for (debug surface). Key bytes come from shared memory (left there by fill_tile) for
 // the first kResidentSubs sub-tiles.
+// The same for a tile of ONE sub-tile, in two halves: the ranks inside the tile (everything that does not depend on other
+// tiles: key counts, the two block scans) are formed BEFORE the block waits for the tiles before it, the index stores after.
+__device__ __forceinline__ void scatter_ranks(const DeviceState& D, BookSmem& sm, unsigned long long& plo, unsigned long long& phi) {
+  const uint32_t kv = sm.skey[threadIdx.x];
+  unsigned long long lo = 0, hi = 0;
+#pragma unroll
+  for (int i = 0; i < kKeysPerThread; ++i) {
+    const uint32_t kb = (kv >> (8 * i)) & 0xff;
+    if (kb != 0xff) {
+      const int s = sort_key_of(D.sort_mode, kb);
+      if (s < 4) lo += 1ull << (16 * s); else hi += 1ull << (16 * (s - 4));
+    }
+  }
+  unsigned long long tot;
+  plo = block_excl_scan64(lo, sm.scan64, tot);
+  phi = 0;
+  if (D.sort_mode == 1) phi = block_excl_scan64(hi, sm.scan64, tot);
+}
+__device__ __forceinline__ void scatter_store(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long plo, unsigned long long phi) {
+  const int vacant_key = D.sort_mode == 1 ? (int)A_VACANT : 3;
+  const uint32_t base = (tile << D.tile_shift) + threadIdx.x * kKeysPerThread;
+  const uint32_t kv = sm.skey[threadIdx.x];
+#pragma unroll
+  for (int i = 0; i < kKeysPerThread; ++i) {
+    const uint32_t kb = (kv >> (8 * i)) & 0xff;
+    if (kb != 0xff) {
+      const int s = sort_key_of(D.sort_mode, kb);
+      uint32_t r;
+      if (s < 4) { r = (uint32_t)((plo >> (16 * s)) & 0xffff); plo += 1ull << (16 * s); }
+      else { r = (uint32_t)((phi >> (16 * (s - 4))) & 0xffff); phi += 1ull << (16 * (s - 4)); }
+      if (s != vacant_key || D.write_vacant) D.indices[(size_t)s * D.N + sm.base[s] + r] = base + i;
+    }
+  }
+}
 __device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm, uint32_t tile) {
   const int vacant_key = D.sort_mode == 1 ? (int)A_VACANT : 3;
   for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
@@ -312,12 +347,13 @@ __device__ __forceinline__ void scatter_tile(const DeviceState& D, BookSmem& sm,
 // Exclusive scan of nsec[slot] in ascending SLOT order (in every sort mode), so that the initializer order — and with
 // it every later slot assignment and PRNG stream — does not depend on thread timing or on the sort mode. A tile's
 // offset `off0` comes from the two-level counters of staged secondaries; a tile that staged nothing is not read at all.
+// nv0: the thread's four nsec bytes of sub-tile 0, loaded by the caller together with its other prologue loads
 __device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t off0,
-                                          uint32_t tile_total, bool overflow) {
+                                          uint32_t tile_total, bool overflow, uint32_t nv0) {
   const uint32_t off_end = off0 + tile_total;
   for (uint32_t sub = 0; sub < D.subs_per_tile && off0 < off_end; ++sub) {
     const uint32_t base = (tile << D.tile_shift) + sub * kSub + threadIdx.x * kKeysPerThread;
-    const uint32_t nv = *reinterpret_cast<const uint32_t*>(D.nsec + base);
+    const uint32_t nv = sub == 0 ? nv0 : *reinterpret_cast<const uint32_t*>(D.nsec + base);
     const uint32_t c = (nv & 0xff) + ((nv >> 8) & 0xff) + ((nv >> 16) & 0xff) + (nv >> 24);   // bytes are 0..2
     uint32_t total;
     uint32_t r = block_excl_scan(c, sm.scan, total);
@@ -412,6 +448,8 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   ControlCarry cc; cc.track_steps = ctl->track_steps; cc.iterations = ctl->iterations; cc.n_logged = ctl->n_logged;   // (used by the last tile's block)
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
   if (threadIdx.x < 12) sm.before[threadIdx.x] = 0;
+  // (the key bytes too: the kernels that write them — the action kernels, the previous fill — are complete; the push is not one)
+  const uint32_t kv0 = *reinterpret_cast<const uint32_t*>(D.akey + ((size_t)tile << D.tile_shift) + threadIdx.x * kKeysPerThread);
   uint32_t prefix, V, tile_vacant;
   tile_prefix(D, sm, D.tile_vac + (size_t)p * D.n_tiles, tile, prefix, V, tile_vacant);
   pdl_prologue();
@@ -422,7 +460,7 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   if (threadIdx.x == 8) D.tile_sec[tile] = 0;   // consumed by the push of the previous iteration
   const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
-  const bool keys_read = fill_tile(D, sm, tile, I, plan, prefix, tile_vacant);
+  const bool keys_read = fill_tile(D, sm, tile, I, plan, prefix, tile_vacant, kv0);
   __syncthreads();
   // ---- publish: the tile's rows, its group's rows, what is left of its vacancies; then the stamps the later tiles wait for
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
@@ -455,6 +493,10 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   }
   const bool scatter = n_keys != 0 && (keys_read || D.write_vacant);
   if (!scatter && !is_last) return;
+  // a tile of one sub-tile forms its ranks now, while the tiles before it are still publishing
+  const bool early_ranks = scatter && D.subs_per_tile == 1;
+  unsigned long long plo = 0, phi = 0;
+  if (early_ranks) scatter_ranks(D, sm, plo, phi);
   // ---- wait for the tiles before this one: ONE thread polls the mask of complete groups (a word per 32 groups) and the
   // mask of published tiles of the own group, with a back-off, so that a thousand waiting blocks cost L2 next to nothing;
   // then the per-key counts of whole lower groups come from the group rows, those of the lower tiles of the own group
@@ -515,7 +557,8 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   }
   if (!scatter) return;
   __syncthreads();
-  scatter_tile(D, sm, tile);
+  if (early_ranks) scatter_store(D, sm, tile, plo, phi);
+  else scatter_tile(D, sm, tile);
 }
 
 // ================================================================ k_push: P5 (one block per tile)
@@ -530,6 +573,8 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
   const int32_t error = ctl->error;
   const unsigned long long I = ctl->n_init_fill;
+  // (issued with the loads above and the counters below: one round trip for the whole prologue; 1 KB wasted by a tile that staged nothing)
+  const uint32_t nv0 = *reinterpret_cast<const uint32_t*>(D.nsec + ((size_t)tile << D.tile_shift) + threadIdx.x * kKeysPerThread);
   uint32_t prefix, S, tile_total;
   tile_prefix(D, sm, D.tile_sec, tile, prefix, S, tile_total);
   if (finished) return;
@@ -543,7 +588,7 @@ __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
     ctl->iter = iter + 1;
   }
   if (tile_total == 0) return;
-  push_tile(D, sm, tile, I, prefix, tile_total, overflow);
+  push_tile(D, sm, tile, I, prefix, tile_total, overflow, nv0);
 }
 
 // ================================================================ S9-P: charged / neutral partition of the popped initializers
