@@ -161,6 +161,9 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * switches back if the population grows (the fixed cost of an iteration is exposed at low track counts);
  * results are bit-identical; not used with hits, trace, profile or CEL_SORT_PARTITION. grid_cap: blocks per SM of the action
  * kernels' grids (default 6, measured 1 % faster than 8 on config 2; several contexts sharing the GPU may take a share each).
+ * live_tiles: 1 (default) = the bookkeeping kernels (fill + sort, push) walk only the leading part of the slot array that the
+ * population has reached so far — vacancies are filled in ascending slot order (S9), so everything above is vacant — 0 = the
+ * whole array in every iteration; results are bit-identical (always 0 on the debug surface and with CEL_SORT_PARTITION).
  * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
  * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);

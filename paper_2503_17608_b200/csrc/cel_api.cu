@@ -72,6 +72,7 @@ struct cel_ctx {
   int concurrent = 1;
   int tail = 1; int tail_iters = 256; int tail_enter = 512;   // k_tail: small populations (cel_tail.cuh)
   uint64_t tail_launches = 0;
+  int live_tiles = 1; // option "live_tiles": the bookkeeping kernels walk only the tiles the population has reached (0 = every tile)
   int grid_cap = 6;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
   bool no_pdl_next = false;
@@ -211,13 +212,15 @@ struct Layout {
 
 // bookkeeping tiles (cel_device.cuh): sub-tiles of kSub slots, tiles of 2^shift slots in groups of kGroupTiles
 struct Tiling { uint32_t n_tiles, tile_shift, subs_per_tile, n_groups; };
-uint64_t g_max_tiles_small = 2048, g_max_tiles_large = 4096;   // (cel_set_option "max_tiles": measurement knob)
+uint64_t g_max_tiles_small = 4096, g_max_tiles_large = 8192;
 Tiling make_tiling(uint64_t N, uint64_t max_tiles_override = 0) {
   const uint64_t subs = (N + kSub - 1) / kSub;
   uint32_t spt = 1, shift = 10;
   static_assert(kSub == 1024, "tile_shift assumes 1024-slot sub-tiles");
-  // at most 2048 tiles up to 2^22 slots, 4096 beyond (measured: more, smaller tiles pay only when a block would
-  // otherwise walk many sub-tiles; every block of a bookkeeping kernel costs launch time in the lightly loaded iterations)
+  // 1024-slot tiles up to 2^22 slots (4096 tiles), at most 8192 tiles beyond. Measured with the live-tile bound (blocks above
+  // the population leave at once): 2^22 slots 27.8 ms with 4096 tiles vs 29.8 with 2048; 2^24 slots 29.5 ms with 8192 tiles
+  // vs 34.7 with 4096 and 30.6 with 16384 — a block that walks several sub-tiles does them one after the other, and every
+  // block of a bookkeeping kernel, live or not, costs launch time
   uint64_t max_tiles = N > (1ull << 22) ? g_max_tiles_large : g_max_tiles_small;
   if (max_tiles_override) max_tiles = max_tiles_override;
   if (max_tiles > (uint64_t)kMaxTiles) max_tiles = kMaxTiles;
@@ -503,6 +506,7 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "tail")) c->tail = v ? 1 : 0;
   else if (!std::strcmp(name, "tail_iters")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->tail_iters = (int)v; }
   else if (!std::strcmp(name, "tail_enter")) { if (v < 0 || v > kTailCap) return CEL_ERR_INVALID_ARG; c->tail_enter = (int)v; }
+  else if (!std::strcmp(name, "live_tiles")) { if (v != 0 && v != 1) return CEL_ERR_INVALID_ARG; c->live_tiles = (int)v; }
   else if (!std::strcmp(name, "grid_cap")) { if (v < 1 || v > 32) return CEL_ERR_INVALID_ARG; c->grid_cap = (int)v; }
   else if (!std::strcmp(name, "hits")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->hits_mode = (int)v; }
   else if (!std::strcmp(name, "hit_tally")) c->hit_tally = v ? 1 : 0;
@@ -679,6 +683,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
   int rc = lay_out(c);
   if (rc != CEL_OK) return rc;
   c->D.write_vacant = debug ? 1 : 0;   // the complete permutation is only needed by the parity surface
+  c->D.bound_tiles = (c->live_tiles && !debug && c->D.sort_mode != CEL_SORT_PARTITION) ? 1 : 0;
   cudaStream_t s = c->stream;
   DeviceState& D = c->D;
   // stream-ordered scratch: freed and re-allocated on the stream, never a device-wide sync
@@ -823,6 +828,7 @@ int load_primaries_host(cel_ctx* c, const cel_primary* p, uint64_t n) {
   CEL_CUDA(c, cudaMallocAsync(&c->d_prim, bytes ? bytes : 64, s));
   if (n) CEL_CUDA(c, cudaMemcpyAsync(c->d_prim, c->h_prim, bytes, cudaMemcpyHostToDevice, s));
   k_load_primaries<<<c->n_sm, 256, 0, s>>>(c->D, (const PrimaryRec*)c->d_prim, n);
+  c->no_pdl_next = true;   // (k_fill_sort reads Control::tiles_hi before its dependency wait)
   c->launches += 1;
   CEL_CUDA(c, cudaGetLastError());
   return CEL_OK;
@@ -939,6 +945,7 @@ extern "C" int cel_transport_device(cel_ctx* c, const void* d_primaries, uint64_
   int rc = prepare_run(c, n_events, false);
   if (rc != CEL_OK) return rc;
   k_load_primaries<<<c->n_sm, 256, 0, c->stream>>>(c->D, (const PrimaryRec*)d_primaries, n);
+  c->no_pdl_next = true;   // (k_fill_sort reads Control::tiles_hi before its dependency wait)
   c->launches += 1;
   CEL_CUDA(c, cudaGetLastError());
   return run_loop(c);

@@ -98,8 +98,8 @@ constexpr int kTileThreads = 256;
 constexpr int kKeysPerThread = 4;
 constexpr int kSub = kTileThreads * kKeysPerThread;  // 1024 slots per sub-tile
 constexpr int kGroupTiles = 32;
-constexpr int kMaxGroups = 128;
-constexpr int kMaxTiles = kMaxGroups * kGroupTiles;  // 4096
+constexpr int kMaxGroups = 256;
+constexpr int kMaxTiles = kMaxGroups * kGroupTiles;  // 8192
 constexpr int kRowWords = 16;                        // one group row: 8 action counts, 4 particle-key counts, arrivals, tile mask, pad
 
 // index ranges of the action kernels in the index array (S2); each kernel walks up to two ranges
@@ -121,6 +121,8 @@ struct Control {
   unsigned long long n_init_fill;   // I after the fill of this iteration (= n_init until k_push adds S)
   uint32_t iter_cur;                // k of the running iteration, a copy k_push may read while its block 0 bumps iter
   uint32_t part_charged;            // sort mode 3: charged initializers among the n_take popped in this iteration
+  uint32_t tiles_hi[2];             // [k&1] = live tiles of iteration k: every tile at or above it is entirely vacant (cel_kernels.cuh)
+  uint32_t vac_low[2];              // [k&1] = vacancies below tiles_hi[(k-1)&1] when iteration k begins
   // hit transfer (option "hits")
   unsigned long long n_hits;        // hit records appended to the device batch buffer since the batch began
   unsigned long long hits_mark[2];  // [k&1] = records already streamed to the host when iteration k's flush starts
@@ -144,6 +146,7 @@ struct DeviceState {
   int sort_mode;          // 0 none, 1 by action, 2 by particle, 3 partition (CEL_SORT_BY_ACTION_REUSE is 1 here, with reuse = 1)
   int reuse;              // S9-R: a slot vacated by its interaction takes its first secondary in place
   int write_vacant;       // 1 = also write the indices of vacant slots (complete permutation, debug surface)
+  int bound_tiles;        // 1 = the bookkeeping kernels walk the live tiles only (Control::tiles_hi); 0 = every tile
   int vac_buf_override;   // 0: vacancies created in iteration k go to the counters of parity (k&1)^1; 1 + p: to parity p (k_tail)
   unsigned long long init_capacity;
   uint32_t n_events;

@@ -7,7 +7,7 @@
 //
 // One 256-thread block per tile of 2^tile_shift consecutive slots. What makes a single pass possible:
 //  * the action kernels keep per-tile counters of vacancies created and secondaries staged (integer atomics), so a
-//    block gets its exclusive prefix from one strided read of <= 4096 counters — no counting pass, no look-back chain;
+//    block gets its exclusive prefix from one strided read of the live tiles' counters (<= 8192) — no counting pass, no look-back chain;
 //  * the index array is kept in REGIONS of N entries, one per sort key: region k holds the slots of key k in ascending
 //    order from k*N, so where a tile writes depends only on the tiles BEFORE it (their per-key counts), never on
 //    totals. A block publishes its tile's histogram (own row + atomics on its group's row), then waits for the tiles
@@ -112,22 +112,33 @@ __device__ __forceinline__ uint32_t real_slots_in_tile(const DeviceState& D, uin
   const unsigned long long lo = (unsigned long long)tile << D.tile_shift, hi = lo + (1ull << D.tile_shift);
   return lo >= D.N ? 0u : (uint32_t)((hi < D.N ? hi : (unsigned long long)D.N) - lo);
 }
-__device__ __forceinline__ uint32_t tiles_in_group(const DeviceState& D, uint32_t g) {
+__device__ __forceinline__ uint32_t tiles_in_group(uint32_t n_tiles, uint32_t g) {
   const uint32_t lo = g * kGroupTiles;
-  return lo >= D.n_tiles ? 0u : min((uint32_t)kGroupTiles, D.n_tiles - lo);
+  return lo >= n_tiles ? 0u : min((uint32_t)kGroupTiles, n_tiles - lo);
+}
+// slots of the first t tiles
+__device__ __forceinline__ uint32_t slots_below_tile(const DeviceState& D, uint32_t t) {
+  const unsigned long long s = (unsigned long long)t << D.tile_shift;
+  return s < D.N ? (uint32_t)s : D.N;
 }
 
-// Exclusive prefix of a per-tile counter by one block: the sum over the tiles before `tile`, the grand total and the tile's
-// own counter. Threads stride over all the counters (n_tiles <= 4096: at most 16 loads per thread, issued back to back before
-// the first use: one L2 round trip). Uses sm.part; ends with a barrier.
-__device__ __forceinline__ void tile_prefix(const DeviceState& D, BookSmem& sm, const uint32_t* tile_cnt, uint32_t tile,
+// Exclusive prefix of a per-tile counter by one block: the sum over the tiles before `tile`, the total and the tile's own
+// counter, over the first n counters (the live tiles, below). Threads stride over them (n <= 8192: at most 32 loads per
+// thread, issued back to back before the first use: one L2 round trip). Uses sm.part; a second call needs a barrier first.
+//
+// Live tiles (Control::tiles_hi): vacancies are filled in ascending slot order, so the tracks of a run occupy a prefix of
+// the slot array whose end only moves up when the population outgrows it; every tile at or above tiles_hi[k & 1] is
+// entirely vacant throughout iteration k, its counters still hold what k_reset_state wrote, and its blocks leave at once.
+// k_push of iteration k-1 sets the bound for iteration k from the stack height: the fill takes min(V, I) vacancies, the
+// first vac_low of them below the old bound, the rest in the consecutive vacant slots above it.
+__device__ __forceinline__ void tile_prefix(BookSmem& sm, const uint32_t* tile_cnt, uint32_t n, uint32_t tile,
                                             uint32_t& prefix, uint32_t& total, uint32_t& own) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   uint32_t before = 0, all = 0, mine = 0;
-  for (uint32_t i0 = 0; i0 < D.n_tiles; i0 += 4 * kTileThreads) {
+  for (uint32_t i0 = 0; i0 < n; i0 += 4 * kTileThreads) {
     uint32_t v[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { const uint32_t i = i0 + u * kTileThreads + threadIdx.x; v[u] = i < D.n_tiles ? __ldcg(tile_cnt + i) : 0u; }
+    for (int u = 0; u < 4; ++u) { const uint32_t i = i0 + u * kTileThreads + threadIdx.x; v[u] = i < n ? __ldcg(tile_cnt + i) : 0u; }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
       const uint32_t i = i0 + u * kTileThreads + threadIdx.x;
@@ -170,6 +181,33 @@ __device__ __forceinline__ uint32_t filled_by_plan(uint32_t v, uint32_t prefix, 
   const uint32_t hs = max(prefix, pl.high_start);
   return lo + (end > hs ? end - hs : 0u);
 }
+// adds the action histogram (and, sorted by particle, the sort-key histogram) of this thread's 4 key bytes to sm.act / sm.hist
+__device__ __forceinline__ void add_key_histograms(const DeviceState& D, BookSmem& sm, uint32_t kv) {
+  // histograms of this thread's 4 keys, 8 x 8-bit packed (padding bytes 0xff are skipped)
+  uint32_t a_lo = 0, a_hi = 0, s_lo = 0;
+#pragma unroll
+  for (int i = 0; i < kKeysPerThread; ++i) {
+    const uint32_t kb = (kv >> (8 * i)) & 0xff;
+    if (kb != 0xff) {
+      const uint32_t a = kb & 0xf;
+      if (a < 4) a_lo += 1u << (8 * a); else a_hi += 1u << (8 * (a - 4));
+      if (D.sort_mode == 2) s_lo += 1u << (8 * sort_key_of(2, kb));
+    }
+  }
+  // warp totals: at most 128 per key, so the 8-bit fields cannot carry
+  a_lo = __reduce_add_sync(0xffffffffu, a_lo); a_hi = __reduce_add_sync(0xffffffffu, a_hi);
+  if (D.sort_mode == 2) s_lo = __reduce_add_sync(0xffffffffu, s_lo);
+  {  // lanes 0-7 add the warp's count of key `lane`
+    const uint32_t lane = threadIdx.x & 31;
+    if (lane < 8) {
+      const uint32_t sh = 8 * (lane & 3);
+      const uint32_t a = ((lane < 4 ? a_lo : a_hi) >> sh) & 0xff;
+      if (a) atomicAdd(&sm.act[lane], a);
+      if (D.sort_mode == 2 && lane < 4) { const uint32_t h = (s_lo >> sh) & 0xff; if (h) atomicAdd(&sm.hist[lane], h); }
+    }
+  }
+}
+
 // returns true if the tile's key bytes were read (false: the tile is entirely vacant and gets no fill)
 // kv0: the key bytes of the thread's four slots in sub-tile 0, loaded by the caller ahead of time
 __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, const FillPlan pl,
@@ -230,29 +268,52 @@ __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, ui
     } else if (sub < (uint32_t)kResidentSubs) {
       skey[threadIdx.x] = kv;
     }
-    // histograms of this thread's 4 keys, 8 x 8-bit packed (padding bytes 0xff are skipped)
-    uint32_t a_lo = 0, a_hi = 0, s_lo = 0;
+    add_key_histograms(D, sm, kv);
+  }
+  return true;
+}
+
+// ---- the tiles the population grows into (at or above the live tiles of the previous iteration: entirely vacant, so the
+// fills that reach them land on CONSECUTIVE slots: slot `below + m` takes init[I-1-(vac_low+m)], m < n_high). One block per
+// tile would copy its 1024+ records a few per thread and round trip, while the blocks above the live tiles have nothing
+// to do: those copy the records (grown_copy, a grid-stride loop, about one record half per thread), and the tile's own
+// block only reads the 8-byte meta words it needs for the key bytes and the histograms (fill_grown_tile).
+__device__ __forceinline__ void grown_copy(const DeviceState& D, unsigned long long I, uint32_t vac_low, uint32_t below,
+                                           uint32_t n_high, uint32_t helper, uint32_t n_helpers) {
+  for (unsigned long long w = (unsigned long long)helper * kTileThreads + threadIdx.x; w < 2ull * n_high; w += (unsigned long long)n_helpers * kTileThreads) {
+    const uint32_t m = (uint32_t)(w >> 1);
+    const unsigned long long src = I - 1ull - (unsigned long long)(vac_low + m);
+    const uint32_t slot = below + m;
+    if (w & 1) store_b(D.stB + slot, load_b(D.initB + src));
+    else store_a(D.stA + slot, load_a(D.initA + src));
+  }
+}
+__device__ __forceinline__ bool fill_grown_tile(const DeviceState& D, BookSmem& sm, uint32_t tile, unsigned long long I, uint32_t vac_low,
+                                                uint32_t below, uint32_t n_high, uint32_t kv0) {
+  const uint32_t tile_base = tile << D.tile_shift;
+  if (tile_base - below >= n_high) {   // no fill reaches it (the bound is a whole tile count)
+    if (threadIdx.x == 0) { sm.act[A_VACANT] = real_slots_in_tile(D, tile); if (D.sort_mode == 2) sm.hist[3] = sm.act[A_VACANT]; }
+    return false;
+  }
+  for (uint32_t sub = 0; sub < D.subs_per_tile; ++sub) {
+    const uint32_t base = tile_base + sub * kSub + threadIdx.x * kKeysPerThread;
+    uint32_t kv = sub == 0 ? kv0 : *reinterpret_cast<const uint32_t*>(D.akey + base);
+    unsigned long long meta[kKeysPerThread];
 #pragma unroll
-    for (int i = 0; i < kKeysPerThread; ++i) {
-      const uint32_t kb = (kv >> (8 * i)) & 0xff;
-      if (kb != 0xff) {
-        const uint32_t a = kb & 0xf;
-        if (a < 4) a_lo += 1u << (8 * a); else a_hi += 1u << (8 * (a - 4));
-        if (D.sort_mode == 2) s_lo += 1u << (8 * sort_key_of(2, kb));
-      }
+    for (int i = 0; i < kKeysPerThread; ++i) {   // (slots below `below + n_high` are real slots)
+      const uint32_t m = base + i - below;
+      meta[i] = m < n_high ? reinterpret_cast<const unsigned long long*>(D.initB + (I - 1ull - (unsigned long long)(vac_low + m)))[3] : 0ull;
     }
-    // warp totals: at most 128 per key, so the 8-bit fields cannot carry
-    a_lo = __reduce_add_sync(0xffffffffu, a_lo); a_hi = __reduce_add_sync(0xffffffffu, a_hi);
-    if (D.sort_mode == 2) s_lo = __reduce_add_sync(0xffffffffu, s_lo);
-    {  // lanes 0-7 add the warp's count of key `lane`
-      const uint32_t lane = threadIdx.x & 31;
-      if (lane < 8) {
-        const uint32_t sh = 8 * (lane & 3);
-        const uint32_t a = ((lane < 4 ? a_lo : a_hi) >> sh) & 0xff;
-        if (a) atomicAdd(&sm.act[lane], a);
-        if (D.sort_mode == 2 && lane < 4) { const uint32_t h = (s_lo >> sh) & 0xff; if (h) atomicAdd(&sm.hist[lane], h); }
+    bool any = false;
+#pragma unroll
+    for (int i = 0; i < kKeysPerThread; ++i)
+      if (base + i - below < n_high) {
+        kv = (kv & ~(0xffu << (8 * i))) | ((uint32_t)make_key(meta_action(meta[i]), meta_ptype(meta[i])) << (8 * i));
+        any = true;
       }
-    }
+    if (any) *reinterpret_cast<uint32_t*>(D.akey + base) = kv;
+    if (sub < (uint32_t)kResidentSubs) sm.skey[sub * kTileThreads + threadIdx.x] = kv;
+    add_key_histograms(D, sm, kv);
   }
   return true;
 }
@@ -443,28 +504,71 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   // the group counters of the OTHER parity): `finished`, `iter_cur` and the vacancy counters of parity k&1 were last
   // written by the action kernels / the previous k_fill_sort, which had completed before that kernel let this one start.
   const uint32_t finished = ctl->finished;
-  const uint32_t k = ctl->iter_cur + 1u;          // iter_cur = 0xffffffff after the reset
-  const uint32_t p = k & 1u;
+  uint32_t k = ctl->iter_cur + 1u;                // iter_cur = 0xffffffff after the reset
+  uint32_t p = k & 1u;
+  uint32_t T_prev = ctl->tiles_hi[p ^ 1u];        // live tiles of iteration k-1 (set by k_push of iteration k-2): the counters to read
   ControlCarry cc; cc.track_steps = ctl->track_steps; cc.iterations = ctl->iterations; cc.n_logged = ctl->n_logged;   // (used by the last tile's block)
   if (threadIdx.x < 8) { sm.hist[threadIdx.x] = 0; sm.act[threadIdx.x] = 0; }
   if (threadIdx.x < 12) sm.before[threadIdx.x] = 0;
   // (the key bytes too: the kernels that write them — the action kernels, the previous fill — are complete; the push is not one)
-  const uint32_t kv0 = *reinterpret_cast<const uint32_t*>(D.akey + ((size_t)tile << D.tile_shift) + threadIdx.x * kKeysPerThread);
-  uint32_t prefix, V, tile_vacant;
-  tile_prefix(D, sm, D.tile_vac + (size_t)p * D.n_tiles, tile, prefix, V, tile_vacant);
+  const uint8_t* const key_ptr = D.akey + ((size_t)tile << D.tile_shift) + threadIdx.x * kKeysPerThread;
+  bool was_live = tile < T_prev;                  // block-uniform
+  uint32_t kv0 = 0, prefix = 0, V = 0, tile_vacant = 0;
+  if (was_live) {
+    kv0 = *reinterpret_cast<const uint32_t*>(key_ptr);
+    tile_prefix(sm, D.tile_vac + (size_t)p * D.n_tiles, T_prev, tile, prefix, V, tile_vacant);
+  }
   pdl_prologue();
   const uint32_t n_charged = ctl->part_charged;
   const unsigned long long I = ctl->n_init;
+  // A block above the live tiles may start after the block of the last live tile has already advanced iter_cur (the grid
+  // need not be resident at once, and the live tiles wait only for each other): `iter`, which the push before this
+  // kernel set and nothing changes until the next push, decides; such a block redoes the little it did.
+  const uint32_t k_now = ctl->iter;
+  if (k_now != k) {
+    k = k_now; p = k & 1u;
+    T_prev = ctl->tiles_hi[p ^ 1u];
+    was_live = tile < T_prev;
+    if (was_live) {   // (cannot be: a live tile's block has read iter_cur before the last live tile's block got past its wait for it)
+      __syncthreads();
+      kv0 = *reinterpret_cast<const uint32_t*>(key_ptr);
+      tile_prefix(sm, D.tile_vac + (size_t)p * D.n_tiles, T_prev, tile, prefix, V, tile_vacant);
+    }
+  }
+  const uint32_t T = ctl->tiles_hi[p];            // live tiles of this iteration (k_push of iteration k-1)
+  const uint32_t vac_low = ctl->vac_low[p];       // vacancies below T_prev (the same sum the blocks below T_prev just formed)
   if (finished) return;
+  // the rows and the mask the next iteration adds into (last used by iteration k-1, which is complete)
+  if (tile < D.n_groups && threadIdx.x >= 32 && threadIdx.x < 32 + kRowWords) group_row(D, p ^ 1u, tile)[threadIdx.x - 32] = 0u;
+  if (tile == 0 && threadIdx.x >= 64 && threadIdx.x < 64 + kMaxGroups / 32) D.group_mask[(p ^ 1u) * (kMaxGroups / 32) + (threadIdx.x - 64)] = 0u;
+  const uint32_t below = slots_below_tile(D, T_prev);
+  if (!was_live) V = vac_low;                     // (everything from T_prev up is vacant)
+  V += D.N - below;
+  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
+  // fills that land above the live tiles of the previous iteration, and who copies their records: the blocks that have
+  // nothing else to do, when there are at least as many of them as tiles to grow into (block-uniform, the same in every block)
+  const uint32_t n_high = n_take > vac_low ? n_take - vac_low : 0u;
+  const uint32_t n_helpers = D.n_tiles - T;
+  const bool helpers_copy = D.bound_tiles && T > T_prev && n_high != 0u && n_helpers >= T - T_prev;
+  if (tile >= T) {                                // entirely vacant, and nothing reaches it in this iteration
+    if (helpers_copy) { const TraceScope<K_FILL_SORT, TRACE> trace(D, k); grown_copy(D, I, vac_low, below, n_high, tile - T, n_helpers); }
+    return;
+  }
+  if (!was_live) {   // a tile the population grows into: its prefix is a closed form
+    kv0 = *reinterpret_cast<const uint32_t*>(key_ptr);
+    tile_vacant = real_slots_in_tile(D, tile);
+    prefix = vac_low + (slots_below_tile(D, tile) - below);
+    __syncthreads();   // (the zeroed histograms; the blocks below T_prev passed the barriers of tile_prefix)
+  }
   const TraceScope<K_FILL_SORT, TRACE> trace(D, k);
   if (threadIdx.x == 8) D.tile_sec[tile] = 0;   // consumed by the push of the previous iteration
-  const uint32_t n_take = (unsigned long long)V < I ? V : (uint32_t)I;
   const FillPlan plan = D.sort_mode == 3 ? partition_plan(n_take, V, n_charged) : plain_plan(n_take);
-  const bool keys_read = fill_tile(D, sm, tile, I, plan, prefix, tile_vacant, kv0);
+  const bool keys_read = (!was_live && helpers_copy) ? fill_grown_tile(D, sm, tile, I, vac_low, below, n_high, kv0)
+                                                     : fill_tile(D, sm, tile, I, plan, prefix, tile_vacant, kv0);
   __syncthreads();
   // ---- publish: the tile's rows, its group's rows, what is left of its vacancies; then the stamps the later tiles wait for
   const int n_keys = D.sort_mode == 1 ? 8 : (D.sort_mode == 2 ? 4 : 0);
-  const bool is_last = tile == D.n_tiles - 1u;
+  const bool is_last = tile == T - 1u;
   {
     uint32_t* row = group_row(D, p, g);
     if (threadIdx.x < 8) {
@@ -478,14 +582,11 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
     } else if (threadIdx.x == 12) {
       D.tile_vac[(size_t)(p ^ 1u) * D.n_tiles + tile] = tile_vacant - filled_by_plan(tile_vacant, prefix, plan);
     }
-    if (tile < D.n_groups && threadIdx.x >= 32 && threadIdx.x < 32 + kRowWords)   // the row the next iteration adds into
-      group_row(D, p ^ 1u, tile)[threadIdx.x - 32] = 0u;
-    if (tile == 0 && threadIdx.x >= 64 && threadIdx.x < 64 + kMaxGroups / 32) D.group_mask[(p ^ 1u) * (kMaxGroups / 32) + (threadIdx.x - 64)] = 0u;
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) {   // the two bits the later tiles poll: "this tile has published", "this group is complete"
       atomicOr(row + 13, 1u << (tile - tg0));
-      if (atomicAdd(row + 12, 1u) == tiles_in_group(D, g) - 1u) {
+      if (atomicAdd(row + 12, 1u) == tiles_in_group(T, g) - 1u) {
         __threadfence();
         atomicOr(D.group_mask + p * (kMaxGroups / 32) + g / 32, 1u << (g & 31u));
       }
@@ -547,11 +648,12 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
     __syncthreads();
   }
   if (threadIdx.x < 8) sm.base[threadIdx.x] = sm.before[D.sort_mode == 2 ? 8 + (threadIdx.x & 3) : threadIdx.x];
-  if (is_last && threadIdx.x == 0) {   // every other tile is before this one: totals = before + own
+  if (is_last && threadIdx.x == 0) {   // every other live tile is before this one: totals = before + own (+ the vacant tiles above)
     uint32_t act_total[8], key_total[8];
+    const uint32_t above = D.N - slots_below_tile(D, T);
     for (int i = 0; i < 8; ++i) {
-      act_total[i] = sm.before[i] + sm.act[i];
-      key_total[i] = D.sort_mode == 2 ? (i < 4 ? sm.before[8 + i] + sm.hist[i] : 0u) : act_total[i];
+      act_total[i] = sm.before[i] + sm.act[i] + (i == A_VACANT ? above : 0u);
+      key_total[i] = D.sort_mode == 2 ? (i < 4 ? sm.before[8 + i] + sm.hist[i] + (i == 3 ? above : 0u) : 0u) : act_total[i];
     }
     update_control_after_fill(D, act_total, key_total, n_keys, I - n_take, V, k, cc);
   }
@@ -565,27 +667,55 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
 template <bool TRACE>
 __global__ void __launch_bounds__(kTileThreads) k_push(DeviceState D) {
   __shared__ BookSmem sm;
-  pdl_prologue();
   Control* ctl = D.ctl;
   const uint32_t tile = blockIdx.x;
+  // ---- before the programmatic-dependency wait: what k_fill_sort of this iteration and the kernels before it left (they
+  // were complete before the kernel just before this one — an action kernel — let this one start)
+  const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
+  const unsigned long long I = ctl->n_init_fill;
+  const uint32_t T = ctl->tiles_hi[iter & 1u];     // live tiles of this iteration: nothing was staged above them
+  if (tile >= T) return;
+  pdl_prologue();
   // No "last block" here: every block forms S itself, and block 0 alone updates the control block — it writes only fields
   // that no block of this kernel reads (n_init and iter are read through the copies k_fill_sort left: n_init_fill, iter_cur).
-  const uint32_t finished = ctl->finished, iter = ctl->iter_cur;
   const int32_t error = ctl->error;
-  const unsigned long long I = ctl->n_init_fill;
   // (issued with the loads above and the counters below: one round trip for the whole prologue; 1 KB wasted by a tile that staged nothing)
   const uint32_t nv0 = *reinterpret_cast<const uint32_t*>(D.nsec + ((size_t)tile << D.tile_shift) + threadIdx.x * kKeysPerThread);
   uint32_t prefix, S, tile_total;
-  tile_prefix(D, sm, D.tile_sec, tile, prefix, S, tile_total);
+  tile_prefix(sm, D.tile_sec, T, tile, prefix, S, tile_total);
   if (finished) return;
   const TraceScope<K_PUSH, TRACE> trace(D, iter);
   const bool overflow = error != 0 || I + S > D.init_capacity;
-  if (tile == 0 && threadIdx.x == 0) {
-    ctl->push_total = S;
-    if (I + S > D.init_capacity) ctl->error = -4;  // CEL_ERR_INIT_OVERFLOW (sticky)
-    else if (error == 0) ctl->n_init = I + S;
-    ctl->secondaries += S;
-    ctl->iter = iter + 1;
+  if (tile == 0) {
+    if (threadIdx.x == 0) {
+      ctl->push_total = S;
+      if (I + S > D.init_capacity) ctl->error = -4;  // CEL_ERR_INIT_OVERFLOW (sticky)
+      else if (error == 0) ctl->n_init = I + S;
+      ctl->secondaries += S;
+      ctl->iter = iter + 1;
+    }
+    // the live tiles of the next iteration (see tile_prefix): its fill takes n_take = min(V, I) vacancies in ascending
+    // order, vac_low of them below T, the rest in the consecutive vacant slots above
+    const uint32_t q = (iter + 1u) & 1u;
+    uint32_t unused0, vac_low, unused1;
+    __syncthreads();
+    tile_prefix(sm, D.tile_vac + (size_t)q * D.n_tiles, T, 0u, unused0, vac_low, unused1);
+    if (threadIdx.x == 0) {
+      const uint32_t below = slots_below_tile(D, T);
+      const unsigned long long V = (unsigned long long)vac_low + (D.N - below);
+      const unsigned long long I_next = overflow ? I : I + S;
+      const unsigned long long n_take = V < I_next ? V : I_next;
+      uint32_t T_next = T;
+      if (n_take > vac_low) {
+        const unsigned long long top = (unsigned long long)below + (n_take - vac_low);   // one past the highest slot filled
+        T_next = (uint32_t)((top + (1ull << D.tile_shift) - 1ull) >> D.tile_shift);
+        if (T_next > D.n_tiles) T_next = D.n_tiles;
+        if (T_next < T) T_next = T;
+      }
+      ctl->tiles_hi[q] = T_next;
+      ctl->vac_low[q] = vac_low;
+    }
+    __syncthreads();
   }
   if (tile_total == 0) return;
   push_tile(D, sm, tile, I, prefix, tile_total, overflow, nv0);
@@ -760,7 +890,20 @@ __global__ void k_load_primaries(DeviceState D, const PrimaryRec* prim, unsigned
     store_a(D.initA + i, a);
     store_b(D.initB + i, b);
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) D.ctl->n_init = n;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    D.ctl->n_init = n;
+    // live tiles of iteration 0 (tile_prefix): the first min(n, N) slots; none before it. Unbounded (every tile, always)
+    // for the partition rule, which also fills from the top, and on the debug surface, which wants the vacant indices too
+    uint32_t T0 = D.n_tiles, T_before = D.n_tiles;
+    if (D.bound_tiles) {
+      const unsigned long long take = n < D.N ? n : (unsigned long long)D.N;
+      T0 = (uint32_t)((take + (1ull << D.tile_shift) - 1ull) >> D.tile_shift);
+      if (T0 < 1u) T0 = 1u;
+      T_before = 0u;
+    }
+    D.ctl->tiles_hi[0] = T0; D.ctl->tiles_hi[1] = T_before;
+    D.ctl->vac_low[0] = 0u; D.ctl->vac_low[1] = 0u;
+  }
 }
 
 __global__ void k_unpack(const RecA* A, const RecB* B, TrackRec* out, unsigned long long n, int as_initializer) {
@@ -805,9 +948,10 @@ __global__ void k_reset_state(DeviceState D) {
       RecB b; b.dx = b.dy = b.dz = 0.0; b.meta = make_meta(A_VACANT, 0, 0, -1, 0, 0);
       store_a(D.stA + i, a); store_b(D.stB + i, b);
     }
-    if (i < D.n_tiles) {   // vacancy counters of parity 0 (the fill of iteration 0 reads them); everything else in the scratch is zero
+    if (i < D.n_tiles) {   // vacancy counters of both parities (a tile above the live tiles keeps them); everything else in the scratch is zero
       const unsigned long long lo = i << D.tile_shift, hi = (i + 1) << D.tile_shift;
-      D.tile_vac[i] = (uint32_t)(lo >= D.N ? 0ull : ((hi < D.N ? hi : (unsigned long long)D.N) - lo));
+      const uint32_t real = (uint32_t)(lo >= D.N ? 0ull : ((hi < D.N ? hi : (unsigned long long)D.N) - lo));
+      D.tile_vac[i] = real; D.tile_vac[D.n_tiles + i] = real;
     }
     if (i == 0) D.ctl->iter_cur = 0xffffffffu;   // k_fill_sort forms k = iter_cur + 1 before its dependency wait
   }

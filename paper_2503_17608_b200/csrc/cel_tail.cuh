@@ -29,6 +29,7 @@ struct TailSmem {
   uint32_t scan[kTailThreads / 32 + 2];
   uint32_t cnt[8], cursor[8];
   uint32_t n_live, n_tmp;
+  uint32_t top;                      // one past the highest slot the fills of this launch reached
 };
 
 // exclusive scan over the block's kTailThreads threads; total to every thread. Ends with a barrier.
@@ -115,11 +116,19 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail(DeviceState Din, uint3
   unsigned long long track_steps = ctl->track_steps, iterations = ctl->iterations, secondaries = ctl->secondaries;
   uint32_t n_logged = ctl->n_logged;
 
-  // ---- the live list: every non-vacant slot of the tiles that are not entirely vacant, then sorted
-  if (tid == 0) sm.n_live = 0;
+  // ---- the live list: every non-vacant slot of the live tiles (Control::tiles_hi) that are not entirely vacant, then sorted.
+  // First the list of those tiles (sm.tmp; more than kTailCap of them cannot be: each holds a track), all counters in flight
+  // at once; then their key bytes.
+  const uint32_t T = ctl->tiles_hi[pb];
+  if (tid == 0) { sm.n_live = 0; sm.n_tmp = 0; sm.top = 0; }
   __syncthreads();
-  for (uint32_t t = 0; t < D.n_tiles; ++t) {
-    if (tvac[t] == real_slots_in_tile(D, t)) continue;                       // block-uniform
+  for (uint32_t t = tid; t < T; t += kTailThreads)
+    if (__ldcg(tvac + t) != real_slots_in_tile(D, t)) { const uint32_t at = atomicAdd(&sm.n_tmp, 1u); if (at < (uint32_t)kTailCap) sm.tmp[at] = t; }
+  __syncthreads();
+  const uint32_t n_live_tiles = sm.n_tmp;
+  if (n_live_tiles > (uint32_t)kTailCap) return;   // (cannot happen: live tiles <= live tracks <= ctl->alive; nothing has been changed yet)
+  for (uint32_t j = 0; j < n_live_tiles; ++j) {
+    const uint32_t t = sm.tmp[j];
     const uint32_t base = t << D.tile_shift, end = min(base + (1u << D.tile_shift), D.N);
     for (uint32_t s = base + 4 * tid; s < end; s += 4 * kTailThreads) {
       const uint32_t kv = *reinterpret_cast<const uint32_t*>(D.akey + s);    // padding bytes are 0xff: skipped below by s + i < end
@@ -151,6 +160,7 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail(DeviceState Din, uint3
           store_b(D.stB + slot, b);
           D.akey[slot] = make_key(meta_action(b.meta), meta_ptype(b.meta));
           atomicSub(tvac + (slot >> D.tile_shift), 1u);
+          if (r == n_take - 1u && slot >= sm.top) sm.top = slot + 1u;   // (ascending: the last vacancy taken is the highest; one thread)
           other[r + (slot - r)] = slot;          // merged position of the new slot: r + #{live < slot} = slot's own c(r) = slot - r
         } else {
           store_a(D.stA + slot, load_a(D.initA + src));
@@ -219,9 +229,29 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail(DeviceState Din, uint3
 
   // ---- leave everything as the kernels of cel_kernels.cuh expect it at the start of iteration k
   __syncthreads();
+  // the live tiles as the kernels expect them (cel_kernels.cuh: tile_prefix): now those of the entry, or up to the highest
+  // slot a fill of this launch reached; for the fill of iteration k, what k_push would have set: min(V, I) vacancies in
+  // ascending order, vac_low of them below T_out, the rest in the consecutive vacant slots above
+  uint32_t T_out = (uint32_t)(((unsigned long long)sm.top + (1ull << D.tile_shift) - 1ull) >> D.tile_shift);
+  if (T_out < T) T_out = T;
+  uint32_t T_next = T_out, vac_low;
+  {
+    uint32_t v = 0;
+    for (uint32_t t = tid; t < T_out; t += kTailThreads) v += __ldcg(tvac + t);
+    tail_block_scan(v, sm.scan, vac_low);
+    const uint32_t below = slots_below_tile(D, T_out);
+    const unsigned long long V = (unsigned long long)vac_low + (D.N - below);
+    const unsigned long long n_take = V < I ? V : I;
+    if (n_take > vac_low) {
+      const unsigned long long top = (unsigned long long)below + (n_take - vac_low);
+      T_next = (uint32_t)((top + (1ull << D.tile_shift) - 1ull) >> D.tile_shift);
+      if (T_next > D.n_tiles) T_next = D.n_tiles;
+      if (T_next < T_out) T_next = T_out;
+    }
+  }
   if ((k & 1u) != pb) {   // fill(k) reads the vacancy counters of parity k&1
     uint32_t* dst = D.tile_vac + (size_t)(k & 1u) * D.n_tiles;
-    for (uint32_t t = tid; t < D.n_tiles; t += kTailThreads) dst[t] = tvac[t];
+    for (uint32_t t = tid; t < T_out; t += kTailThreads) dst[t] = tvac[t];
   }
   for (uint32_t i = tid; i < D.n_groups * kRowWords; i += kTailThreads) group_row(D, k & 1u, 0)[i] = 0u;   // the rows fill(k) adds into
   if (tid < kMaxGroups / 32) D.group_mask[(k & 1u) * (kMaxGroups / 32) + tid] = 0u;
@@ -231,6 +261,7 @@ __global__ void __launch_bounds__(kTailThreads, 1) k_tail(DeviceState Din, uint3
     ctl->alive = n_live;   // (an upper bound of the live tracks, as after P1 of the last iteration: what the host's switch looks at)
     ctl->n_init = I; ctl->n_init_fill = I;
     ctl->iter = k; ctl->iter_cur = k - 1u;
+    ctl->tiles_hi[(k & 1u) ^ 1u] = T_out; ctl->tiles_hi[k & 1u] = T_next; ctl->vac_low[k & 1u] = vac_low;
     ctl->track_steps = track_steps; ctl->iterations = iterations; ctl->secondaries = secondaries; ctl->n_logged = n_logged;
     if (finished) ctl->finished = 1;
     if (overflow) ctl->error = -4;   // CEL_ERR_INIT_OVERFLOW (sticky)

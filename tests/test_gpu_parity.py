@@ -464,3 +464,21 @@ def test_tail_kernel_identical(binding, mode):
             assert a["track_steps"] == ref["track_steps"] and a["secondaries"] == ref["secondaries"] and a["iterations"] == ref["iterations"]
         a, _ = run_gpu(binding, w0, tail=1)
         assert a["kernel_launches"] < ref["kernel_launches"]          # the tail form was used
+
+
+@pytest.mark.parametrize("mode", [1, 0, 2, 4])
+def test_live_tiles_identical(binding, mode):
+    """the bookkeeping kernels walk only the tiles the population has reached (option live_tiles, the default;
+    cel_kernels.cuh: tile_prefix): tallies, per-iteration counts and counters are bit-identical to walking every tile in
+    every iteration — while the population grows tile by tile (few primaries in many slots), when it fills the array
+    and the stack takes the rest (5000 slots), with ragged last tiles, and together with the single-block tail form
+    (whose fills move the bound too)"""
+    cases = (W.config2(n_events=3, n_slots=1 << 16, energy=2000.0), W.config2(n_events=3, n_slots=5000, energy=150.0),
+             W.config3(n_events=6, n_slots=(1 << 15) + 77, energy=400.0), W.config4(n_events=2, per_event=4, n_slots=1 << 14))
+    for w0 in cases:
+        w0.sort_mode = mode
+        ref, cref = run_gpu(binding, w0, live_tiles=0, tail=0)
+        for opts in (dict(tail=0), dict(tail=1), dict(tail=1, tail_iters=3, batch=2), dict(tail=0, use_graph=0, batch=3)):
+            a, ca = run_gpu(binding, w0, live_tiles=1, **opts)
+            assert np.array_equal(a["fixed"], ref["fixed"]) and np.array_equal(ca, cref), (w0.name, mode, opts)
+            assert a["track_steps"] == ref["track_steps"] and a["secondaries"] == ref["secondaries"] and a["iterations"] == ref["iterations"]
