@@ -51,7 +51,8 @@ enum {
   CEL_ERR_MAX_ITER = -8,      /* the run did not end within max_iterations */
   CEL_ERR_INTERNAL = -9,      /* a bookkeeping block gave up waiting for the blocks before it (cannot happen when blocks
                                  are dispatched in index order; reported instead of hanging) */
-  CEL_ERR_HIT_OVERFLOW = -10  /* more hit records in one batch of iterations than option hit_capacity (results invalid) */
+  CEL_ERR_HIT_OVERFLOW = -10, /* more hit records in one batch of iterations than option hit_capacity (results invalid) */
+  CEL_ERR_TOO_LARGE = -11     /* cel_reindex_static: more slots than its fixed device scratch holds (CEL_REINDEX_STATIC_MAX_SLOTS) */
 };
 
 /* one effective element per material (S0) */
@@ -204,6 +205,26 @@ int cel_hit_tallies(cel_ctx*, cel_hit_view* out);
  * never reached) keeps {UINT64_MAX, 0}. cel_set_option("trace_ends", 0) stamps the starts only (no atomics at the end
  * of a kernel: the least perturbing form; end_ns stays 0). Synchronises the stream. Errors: INVALID_ARG, NOT_RUN, CUDA. */
 int cel_trace(cel_ctx*, uint64_t* host_out, uint64_t* n_iters);
+
+/* ---- reindexing without allocation (section 3.2 "state_indices"; docs/PHYSICS_SPEC.md S2) ----
+ * For callers that cannot call cudaMalloc (stream capture, tight serving loops, harnesses that forbid it): the stable
+ * counting sort of slot indices by action key that the transport performs in every step iteration, as ONE call that
+ * allocates nothing — no cudaMalloc / cudaFree / cudaMallocAsync, no context: two kernel launches on `cuda_stream`
+ * (stream-ordered; the call does not synchronise). Its per-tile histograms live in a file-scope device array of 128 KB that
+ * every GPU loading the library holds until the process exits, which fixes the maximum: n_slots <=
+ * CEL_REINDEX_STATIC_MAX_SLOTS (2^22), more is CEL_ERR_TOO_LARGE (nothing is launched).
+ *   d_keys    DEVICE, n_slots bytes, 4-byte aligned, caller-owned: key of slot i = d_keys[i] & 7 (the action, 7 = VACANT:
+ *             the low bits of the transport's key byte; higher bits are ignored)
+ *   d_indices DEVICE, n_slots uint32, caller-owned, written: the slots ordered by key, ascending slot order inside a key
+ *   d_offsets DEVICE, 9 uint32, caller-owned, written: offsets[k] = number of slots with a key below k (offsets[8] = n_slots)
+ * All calls on one device share the scratch array: calls that may OVERLAP on the GPU (different streams, graphs in flight
+ * together) race on it and must be serialised by the caller; calls on one stream are safe back to back (no state is carried
+ * from call to call: every counter a call reads it has written first). The first call on a device resolves the array's
+ * device address (cudaGetSymbolAddress, with the caller's current device): make it outside stream capture.
+ * Errors: TOO_LARGE, INVALID_ARG (null or misaligned pointer), CUDA. */
+#define CEL_REINDEX_STATIC_MAX_SLOTS (1ull << 22)
+uint64_t cel_reindex_static_max_slots(void);
+int cel_reindex_static(const uint8_t* d_keys, uint64_t n_slots, uint32_t* d_indices, uint32_t* d_offsets, void* cuda_stream);
 
 /* ---- debug / parity surface (synchronous, not timed) ---- */
 int cel_debug_begin(cel_ctx*, const cel_primary* primaries, uint64_t n, uint32_t n_events); /* load only */

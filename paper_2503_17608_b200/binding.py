@@ -21,7 +21,7 @@ EXPORTS = ["cel_create", "cel_set_stream", "cel_workspace_bytes", "cel_set_works
            "cel_debug_begin", "cel_debug_step", "cel_debug_read_state", "cel_debug_read_indices",
            "cel_debug_n_initializers", "cel_debug_read_initializers", "cel_debug_n_counts", "cel_debug_read_counts",
            "cel_debug_table", "cel_debug_uniforms", "cel_kernel_count", "cel_kernel_name", "cel_kernel_times", "cel_trace", "cel_debug_math",
-           "cel_set_hit_callback", "cel_hit_tallies"]
+           "cel_set_hit_callback", "cel_hit_tallies", "cel_reindex_static", "cel_reindex_static_max_slots"]
 
 
 class cel_material(C.Structure):
@@ -106,6 +106,9 @@ def load_library():
     L.cel_trace.argtypes = [vp, vp, vp]
     L.cel_set_hit_callback.argtypes = [vp, HIT_CALLBACK, vp]
     L.cel_hit_tallies.argtypes = [vp, C.POINTER(cel_hit_view)]
+    L.cel_reindex_static.argtypes = [vp, C.c_uint64, vp, vp, vp]
+    L.cel_reindex_static_max_slots.restype = C.c_uint64
+    L.cel_reindex_static_max_slots.argtypes = []
     _lib = L
     return L
 
@@ -289,6 +292,19 @@ class Context:
         a = np.ascontiguousarray(x, dtype=np.float64); out = np.zeros(len(a))
         self._check(load_library().cel_debug_math(self.h, int(which), _p(a), len(a), _p(out)), "cel_debug_math")
         return out
+
+
+def reindex_static_max_slots():
+    return int(load_library().cel_reindex_static_max_slots())
+
+
+def reindex_static(d_keys_ptr: int, n_slots: int, d_indices_ptr: int, d_offsets_ptr: int, stream: int = 0):
+    """cel_reindex_static (include/cel.h): the by-action reindexing of DEVICE key bytes into DEVICE indices / offsets without
+    any allocation (fixed 128 KB device scratch: n_slots <= 2^22); stream-ordered on `stream`, does not synchronise"""
+    L = load_library()
+    rc = L.cel_reindex_static(C.c_void_p(d_keys_ptr), int(n_slots), C.c_void_p(d_indices_ptr), C.c_void_p(d_offsets_ptr), C.c_void_p(stream))
+    if rc != 0:
+        raise CelError(rc, "cel_reindex_static", L.cel_strerror(rc).decode())
 
 
 def workspace_bytes(n_slots, init_capacity, sort_mode):

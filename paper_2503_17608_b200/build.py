@@ -5,8 +5,8 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcelstep.so")
-SOURCES = ["cel_api.cu"]
-DEPS = ["cel_api.cu", "cel_kernels.cuh", "cel_physics.cuh", "cel_tail.cuh", "cel_device.cuh", os.path.join("..", "..", "include", "cel.h")]
+SOURCES = ["cel_api.cu", "cel_noalloc.cu"]
+DEPS = ["cel_api.cu", "cel_noalloc.cu", "cel_kernels.cuh", "cel_physics.cuh", "cel_tail.cuh", "cel_device.cuh", os.path.join("..", "..", "include", "cel.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-fmad=false", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]
 

@@ -529,6 +529,7 @@ extern "C" const char* cel_strerror(int code) {
     case CEL_ERR_MAX_ITER: return "iteration limit reached";
     case CEL_ERR_INTERNAL: return "internal error: a bookkeeping wait gave up";
     case CEL_ERR_HIT_OVERFLOW: return "hit buffer overflow (option hit_capacity)";
+    case CEL_ERR_TOO_LARGE: return "more slots than the static scratch of cel_reindex_static holds (2^22)";
     default: return "unknown error";
   }
 }
