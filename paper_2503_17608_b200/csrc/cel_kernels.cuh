@@ -224,7 +224,8 @@ __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, ui
     const uint32_t sub_base = (tile << D.tile_shift) + sub * kSub;
     const uint32_t base = sub_base + threadIdx.x * kKeysPerThread;
     uint32_t kv = sub == 0 ? kv0 : *reinterpret_cast<const uint32_t*>(D.akey + base);
-    uint32_t* skey = sm.skey + (sub < (uint32_t)kResidentSubs ? sub : 0u) * kTileThreads;   // (beyond kResidentSubs: scratch only)
+    // (beyond kResidentSubs: scratch only — the upper half of sm.list, which the fill does not use; NOT a resident sub-tile's place)
+    uint32_t* skey = sub < (uint32_t)kResidentSubs ? sm.skey + sub * kTileThreads : sm.list + kSub;
     uint8_t* skey_b = reinterpret_cast<uint8_t*>(skey);
     if (rank0 < rank_end && filled_by_plan(rank_end - rank0, rank0, pl) != 0) {   // block-uniform: this sub-tile may have vacancies to fill
       const uint32_t c = count_vacant4(kv);

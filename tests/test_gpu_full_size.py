@@ -91,3 +91,28 @@ def test_more_than_2048_tiles(binding):
         w.sort_mode = mode
         v, c = run_gpu(binding, w)
         assert np.array_equal(v["fixed"], ref["fixed"]) and np.array_equal(c, ref_counts), mode
+
+
+def test_maximum_slot_counts(binding):
+    """n_slots up to the maximum cel_create accepts (2^28: 8192 bookkeeping tiles of 32 sub-tiles each, 57 GB of workspace):
+    while the array never fills, tallies, counts and counters do not depend on the slot count (S9: ascending fill; S3:
+    histories keyed by slot and iteration), so the runs at 2^26 and 2^28 slots must equal the run at 2^16 bit for bit —
+    in every sort mode (the tiles of more than 4 sub-tiles re-read their key bytes for the scatter)"""
+    def run(n_slots, mode):
+        w = W.config3(n_events=20, n_slots=n_slots, energy=2000.0, seed=11, sort_mode=mode)
+        w.physics["init_capacity"] = 1 << 22
+        v, c = run_gpu(binding, w)
+        return w, v, c
+    refs = {}
+    for mode in (1, 2, 4, 0):
+        w, v, c = run(1 << 16, mode)
+        whole_run_properties(v, c, w)
+        assert c[:, :7].sum(1).max() < (1 << 16) // 4            # the premise, with room to spare
+        refs[mode] = (v, c)
+    for n_slots, modes in (((1 << 26) + 999, (1, 2, 4, 0)), (1 << 28, (1,))):
+        for mode in modes:
+            w, v, c = run(n_slots, mode)
+            ref, cref = refs[mode]
+            assert np.array_equal(v["fixed"], ref["fixed"]), (n_slots, mode)
+            assert np.array_equal(c[:, :7], cref[:, :7]) and v["track_steps"] == ref["track_steps"] and v["secondaries"] == ref["secondaries"], (n_slots, mode)
+            whole_run_properties(v, c, w)

@@ -165,6 +165,25 @@ def test_sort_mode_invariance_bit_exact():
         assert r[2] == res[0][2]
 
 
+def test_results_do_not_depend_on_the_slot_count_while_the_array_never_fills():
+    """an invariant of S9 + S3: vacancies are filled in ascending slot order and a history is keyed by (seed, slot,
+    iteration), so as long as live tracks + initializers never exceed the slots (the stack is emptied by every fill) the
+    slot assignment — and with it every tally, count and counter — is the same whatever n_slots is"""
+    res = []
+    for n_slots in (1024, 1500, 4096):
+        w, o = small_shower(1, n_slots=n_slots, n_events=5, energy=300.0, seed=33)
+        o.transport(w.primaries, w.n_events)
+        c = o.counts()
+        assert (c[:, :7].sum(1).max()) < 1024                   # the premise: the smallest array never fills
+        res.append((o.tallies_fixed(), c[:, :7].copy(), o.counters()))
+    for r in res[1:]:
+        assert np.array_equal(r[0], res[0][0]) and np.array_equal(r[1], res[0][1]) and r[2] == res[0][2]
+    # and it does depend on it once the array fills (the premise is not vacuous)
+    w, o = small_shower(1, n_slots=64, n_events=5, energy=300.0, seed=33)
+    o.transport(w.primaries, w.n_events)
+    assert not np.array_equal(o.tallies_fixed(), res[0][0])
+
+
 @pytest.mark.parametrize("cfg", ["calo", "calo_field", "barrel"])
 def test_energy_conservation_per_event(cfg):
     """pin 5: deposited + escaped = primary energy (+ 2 m_e per primary positron), per event, 1e-9 relative"""
