@@ -165,6 +165,10 @@ int cel_kernel_times(cel_ctx*, double* ms_out, uint64_t* launches_out);
  * live_tiles: 1 (default) = the bookkeeping kernels (fill + sort, push) walk only the leading part of the slot array that the
  * population has reached so far — vacancies are filled in ascending slot order (S9), so everything above is vacant — 0 = the
  * whole array in every iteration; results are bit-identical (always 0 on the debug surface and with CEL_SORT_PARTITION).
+ * max_tiles: at most this many bookkeeping tiles (of 1024 x 2^j slots; default 0 = 1024-slot tiles up to 2^22 slots, at most
+ * 8192 tiles beyond); only before the first transport, and with a caller-provided workspace the padding of the slot arrays to
+ * whole tiles may need up to one tile more than cel_workspace_bytes states (INVALID_ARG then). A test and measurement knob:
+ * results do not depend on it.
  * trace: see cel_trace. (Execution forms that were measured slower and removed — a persistent cooperative kernel, all
  * actions in one launch — are recorded in DESIGN.md section 10.) */
 int cel_set_option(cel_ctx*, const char* name, int64_t value);

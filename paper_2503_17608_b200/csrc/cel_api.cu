@@ -72,6 +72,7 @@ struct cel_ctx {
   int concurrent = 1;
   int tail = 1; int tail_iters = 256; int tail_enter = 512;   // k_tail: small populations (cel_tail.cuh)
   uint64_t tail_launches = 0;
+  int max_tiles = 0;  // option "max_tiles": upper bound of the number of bookkeeping tiles (0 = the default of make_tiling)
   int live_tiles = 1; // option "live_tiles": the bookkeeping kernels walk only the tiles the population has reached (0 = every tile)
   int grid_cap = 6;   // blocks per SM of the action kernels' grids (option "grid_cap": several contexts sharing the GPU take a share each)
   int merge_discrete = 1;   // sort by action: photoelectric + pair + annihilation in one launch (k_discrete)
@@ -239,9 +240,9 @@ int n_index_regions(int sort_mode) {   // regions of N entries in the index arra
   return 0;
 }
 
-Layout make_layout(uint64_t N, uint64_t cap, int sort_mode) {
+Layout make_layout(uint64_t N, uint64_t cap, int sort_mode, uint64_t max_tiles_override = 0) {
   Layout L{};
-  const Tiling tl = make_tiling(N);
+  const Tiling tl = make_tiling(N, max_tiles_override);
   const uint64_t padded = (uint64_t)tl.n_tiles << tl.tile_shift;
   uint64_t o = 0;
   auto take = [&](uint64_t bytes) { uint64_t r = o; o = align_up(o + bytes, 256); return r; };
@@ -268,7 +269,7 @@ uint64_t default_capacity(uint64_t N, uint64_t cap) {
 
 int lay_out(cel_ctx* c) {
   if (c->laid_out) return CEL_OK;
-  const Layout L = make_layout(c->n_slots, c->D.init_capacity, c->user_sort_mode);
+  const Layout L = make_layout(c->n_slots, c->D.init_capacity, c->user_sort_mode, (uint64_t)c->max_tiles);
   if (!c->workspace) {
     CEL_CUDA(c, cudaMalloc(&c->workspace, L.total));
     c->workspace_bytes = L.total; c->own_workspace = true;
@@ -506,6 +507,12 @@ extern "C" int cel_set_option(cel_ctx* c, const char* name, int64_t v) {
   else if (!std::strcmp(name, "tail")) c->tail = v ? 1 : 0;
   else if (!std::strcmp(name, "tail_iters")) { if (v < 1 || v > (1 << 20)) return CEL_ERR_INVALID_ARG; c->tail_iters = (int)v; }
   else if (!std::strcmp(name, "tail_enter")) { if (v < 0 || v > kTailCap) return CEL_ERR_INVALID_ARG; c->tail_enter = (int)v; }
+  else if (!std::strcmp(name, "max_tiles")) {   // before the first run only: the slot arrays are padded to whole tiles
+    if (v < 0 || v > kMaxTiles || c->laid_out) return CEL_ERR_INVALID_ARG;
+    c->max_tiles = (int)v;
+    const Tiling tl = make_tiling(c->n_slots, (uint64_t)v);
+    c->D.n_tiles = tl.n_tiles; c->D.n_groups = tl.n_groups; c->D.tile_shift = tl.tile_shift; c->D.subs_per_tile = tl.subs_per_tile;
+  }
   else if (!std::strcmp(name, "live_tiles")) { if (v != 0 && v != 1) return CEL_ERR_INVALID_ARG; c->live_tiles = (int)v; }
   else if (!std::strcmp(name, "grid_cap")) { if (v < 1 || v > 32) return CEL_ERR_INVALID_ARG; c->grid_cap = (int)v; }
   else if (!std::strcmp(name, "hits")) { if (v < 0 || v > 2) return CEL_ERR_INVALID_ARG; c->hits_mode = (int)v; }

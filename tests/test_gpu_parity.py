@@ -66,12 +66,14 @@ def check_integer_work_self_consistent(ctx, st, sort_mode, where=""):
         assert np.all(np.diff(seg.astype(np.int64)) > 0), (where, "stable within key", k)
 
 
-def lockstep(binding, w, n_iter, must_match, min_agreed=None):
+def lockstep(binding, w, n_iter, must_match, min_agreed=None, **opts):
     """step both sides together; integer work bit-exact, floating state within 1e-12 and the tallies within the first-step
     deposit tolerance (A24) for the first `must_match` iterations at least. The first later disagreement must be a
     handful of float-driven decision flips (a few slots), not an indexing error; after it the GPU's integer work is still
     checked for self-consistency. Returns how many iterations agreed."""
     ctx = binding.from_workload(w)
+    for name, value in opts.items():
+        ctx.set_option(name, value)
     o = make_oracle(w)
     ctx.begin(w.primaries, w.n_events); o.begin(w.primaries, w.n_events)
     e_max = float(w.primaries["energy"].max()) if len(w.primaries) else 1.0
@@ -482,3 +484,19 @@ def test_live_tiles_identical(binding, mode):
             a, ca = run_gpu(binding, w0, live_tiles=1, **opts)
             assert np.array_equal(a["fixed"], ref["fixed"]) and np.array_equal(ca, cref), (w0.name, mode, opts)
             assert a["track_steps"] == ref["track_steps"] and a["secondaries"] == ref["secondaries"] and a["iterations"] == ref["iterations"]
+
+
+@pytest.mark.parametrize("mode", [1, 0, 2, 3, 4])
+def test_tiles_of_many_sub_tiles(binding, mode):
+    """above 2^25 slots a bookkeeping tile has more than four 1024-slot sub-tiles, of which only four keep their key bytes
+    in shared memory between the fill and the scatter. Option max_tiles makes such tiles at a size the oracle steps
+    through: 3 tiles of 16 sub-tiles (ragged), in lockstep with the oracle while the array fills up and the fills reach
+    every sub-tile (and, partition rule, the top of the array), then whole runs against the default tiling"""
+    w = W.config3(n_events=150, n_slots=40000 + 321, energy=3000.0, seed=19, sort_mode=mode)
+    assert lockstep(binding, w, 110, must_match=4, max_tiles=3) >= 4
+    ref, cref = run_gpu(binding, w)
+    assert cref[:, :7].sum(1).max() == w.n_slots                     # the array does fill
+    for opts in (dict(max_tiles=3), dict(max_tiles=1), dict(max_tiles=7, live_tiles=0, tail=0)):
+        a, ca = run_gpu(binding, w, **opts)
+        assert np.array_equal(a["fixed"], ref["fixed"]) and np.array_equal(ca, cref), (mode, opts)
+        assert a["track_steps"] == ref["track_steps"] and a["secondaries"] == ref["secondaries"] and a["iterations"] == ref["iterations"]
