@@ -245,23 +245,20 @@ __device__ __forceinline__ bool fill_tile(const DeviceState& D, BookSmem& sm, ui
       // cooperative copy: work item w = (record, half); half 0 = RecA, half 1 = RecB (+ the key byte).
       // (Tried: two passes in flight per thread through cp.async landing slots in shared memory — 16 KB more shared
       // memory per block cost more in lost overlap with the neighbouring kernels than the pipelining gained: +7 %.)
-      for (uint32_t w = threadIdx.x; w < 2 * nf; w += kTileThreads) {
-        const uint32_t m = w >> 1;
+      for (uint32_t m = threadIdx.x; m < nf; m += kTileThreads) {   // one record per thread and pass: both halves in flight together
         const uint32_t item = m < n_lo ? m : hi_begin + (m - n_lo);
         const uint32_t slot = sm.list[item];
         const uint32_t rank = rank0 + item;
         uint32_t pop = rank;                                 // plain rule: rank r takes init[I-1-r]
         if (pl.partition) pop = D.indices[rank < pl.low_n ? rank : pl.n_take - 1u - (pl.V - 1u - rank)];
         const unsigned long long src = I - 1ull - (unsigned long long)pop;
-        if (w & 1) {
-          const RecB b = load_b(D.initB + src);
-          store_b(D.stB + slot, b);
-          const uint8_t key = make_key(meta_action(b.meta), meta_ptype(b.meta));
-          D.akey[slot] = key;
-          skey_b[slot - sub_base] = key;
-        } else {
-          store_a(D.stA + slot, load_a(D.initA + src));
-        }
+        const RecB b = load_b(D.initB + src);
+        const RecA a = load_a(D.initA + src);
+        store_b(D.stB + slot, b);
+        const uint8_t key = make_key(meta_action(b.meta), meta_ptype(b.meta));
+        D.akey[slot] = key;
+        skey_b[slot - sub_base] = key;
+        store_a(D.stA + slot, a);
       }
       __syncthreads();
       kv = skey[threadIdx.x];
@@ -431,12 +428,13 @@ __device__ __forceinline__ void push_tile(const DeviceState& D, BookSmem& sm, ui
     }
     __syncthreads();
     if (!overflow) {
-      for (uint32_t w = threadIdx.x; w < 2 * total; w += kTileThreads) {
-        const uint32_t item = w >> 1;
+      for (uint32_t item = threadIdx.x; item < total; item += kTileThreads) {   // one record per thread and pass: both halves in flight
         const uint32_t src = sm.list[item];
         const unsigned long long dst = I + (unsigned long long)(off0 + item);
-        if (w & 1) store_b(D.initB + dst, load_b(D.secB + src));
-        else store_a(D.initA + dst, load_a(D.secA + src));
+        const RecB rb = load_b(D.secB + src);
+        const RecA ra = load_a(D.secA + src);
+        store_b(D.initB + dst, rb);
+        store_a(D.initA + dst, ra);
       }
     }
     off0 += total;
