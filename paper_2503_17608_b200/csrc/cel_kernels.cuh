@@ -597,27 +597,25 @@ __global__ void __launch_bounds__(kTileThreads, 8) k_fill_sort(DeviceState D) {
   const bool early_ranks = scatter && D.subs_per_tile == 1;
   unsigned long long plo = 0, phi = 0;
   if (early_ranks) scatter_ranks(D, sm, plo, phi);
-  // ---- wait for the tiles before this one: ONE thread polls the mask of complete groups (a word per 32 groups) and the
-  // mask of published tiles of the own group, with a back-off, so that a thousand waiting blocks cost L2 next to nothing;
-  // then the per-key counts of whole lower groups come from the group rows, those of the lower tiles of the own group
-  // from their own rows, all loads in flight together
-  if (threadIdx.x == 0) {
-    bool stuck = false;
+  // ---- wait for the tiles before this one: ONE warp polls the mask of complete groups (a word per 32 groups, a lane each)
+  // and the mask of published tiles of the own group, all words in flight together, with a back-off, so that a thousand
+  // waiting blocks cost L2 next to nothing; then the per-key counts of whole lower groups come from the group rows, those
+  // of the lower tiles of the own group from their own rows, all loads in flight together
+  if (threadIdx.x < 32) {   // warp 0: lane w polls word w of the group mask (<= 8 words), lane 31 the own group's tile mask — one
+    const uint32_t lane = threadIdx.x;                         // round trip when everything before has already published
+    const uint32_t* word = nullptr; uint32_t want = 0;
+    if (lane * 32u < g) { word = D.group_mask + p * (kMaxGroups / 32) + lane; want = g - lane * 32u >= 32u ? 0xffffffffu : (1u << (g - lane * 32u)) - 1u; }
+    else if (lane == 31) { word = group_row(D, p, g) + 13; want = (1u << (tile - tg0)) - 1u; }
+    static_assert(kMaxGroups / 32 <= 31, "one lane per word of the group mask, lane 31 for the tile mask");
     uint32_t spins = 0;
-    const uint32_t ns = 100;   // one polling thread per block: a short, fixed pause costs L2 nothing and keeps the wake-up latency low
-    for (uint32_t w = 0; w * 32u < g && !stuck; ++w) {
-      const uint32_t want = g - w * 32u >= 32u ? 0xffffffffu : (1u << (g - w * 32u)) - 1u;
-      while ((load_acquire(D.group_mask + p * (kMaxGroups / 32) + w) & want) != want) {
-        if (++spins > kSpinLimit) { stuck = true; break; }
-        __nanosleep(ns);
-      }
-    }
-    const uint32_t want_t = (1u << (tile - tg0)) - 1u;
-    while (!stuck && (load_acquire(group_row(D, p, g) + 13) & want_t) != want_t) {
-      if (++spins > kSpinLimit) { stuck = true; break; }
+    const uint32_t ns = 100;   // one polling warp per block: a short, fixed pause costs L2 nothing and keeps the wake-up latency low
+    bool ok = want == 0;
+    while (true) {
+      if (!ok) ok = (load_acquire(word) & want) == want;
+      if (__all_sync(0xffffffffu, ok)) break;
+      if (++spins > kSpinLimit) { if (lane == 0) ctl->error = -9; break; }   // CEL_ERR_INTERNAL (sticky)
       __nanosleep(ns);
     }
-    if (stuck) ctl->error = -9;   // CEL_ERR_INTERNAL (sticky)
   }
   __syncthreads();
   {
