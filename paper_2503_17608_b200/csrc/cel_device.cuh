@@ -371,22 +371,30 @@ __device__ __forceinline__ double distance_to_boundary(const Params& P, double x
     if (sx <= sy) { which = HIT_X; return sx; }
     which = HIT_Y; return sy;
   }
+  // The same filter for the cylinders (no square root, no division for a surface the step certainly does not reach): along
+  // the ray the squared radius q(s) = r^2 + 2 b s + a s^2 is convex, so on [0, s_lim] it stays below q(s_lim) — the outer
+  // cylinder is out of reach when q(s_lim) < rho^2 (1 - 1e-9) — and above r^2 + 2 b s_lim (b < 0) — the inner one is out
+  // of reach when that exceeds rho^2 (1 + 1e-9). Most chord substeps of a track curling in a wide gap end there.
   double a = dx * dx + dy * dy;
   double b = x * dx + y * dy;
   double r2 = x * x + y * y;
   double s_in = CEL_INF, s_out = CEL_INF, s_z = CEL_INF;
+  const bool filter = s_lim < 1e300;
   if (a != 0.0) {
     {
       double rho = __ldg(P.bounds + vol + 1);
       if (surf == vol + 1) {
         s_out = (b >= 0.0) ? 0.0 : -2.0 * b / a;
+        s_out = clamp0(s_out);
       } else {
         double c = r2 - rho * rho;
-        double D = b * b - a * c;
-        if (D < 0.0) D = 0.0;
-        s_out = (b > 0.0) ? -c / (b + sqrt(D)) : (-b + sqrt(D)) / a;
+        if (!(filter && c < 0.0 && c + (2.0 * b + a * s_lim) * s_lim < -1e-9 * (rho * rho))) {
+          double D = b * b - a * c;
+          if (D < 0.0) D = 0.0;
+          s_out = (b > 0.0) ? -c / (b + sqrt(D)) : (-b + sqrt(D)) / a;
+          s_out = clamp0(s_out);
+        }
       }
-      s_out = clamp0(s_out);
     }
     if (vol > 0) {
       double rho = __ldg(P.bounds + vol);
@@ -394,13 +402,15 @@ __device__ __forceinline__ double distance_to_boundary(const Params& P, double x
         if (b < 0.0) s_in = 0.0;
       } else if (b < 0.0) {
         double c = r2 - rho * rho;
-        double D = b * b - a * c;
-        if (D > 0.0) s_in = clamp0(c / (-b + sqrt(D)));
+        if (!(filter && c + 2.0 * b * s_lim > 1e-9 * (rho * rho))) {
+          double D = b * b - a * c;
+          if (D > 0.0) s_in = clamp0(c / (-b + sqrt(D)));
+        }
       }
     }
   }
-  if (dz > 0.0) s_z = clamp0((P.half_z - z) / dz);
-  else if (dz < 0.0) s_z = clamp0((-P.half_z - z) / dz);
+  if (dz > 0.0) s_z = filter ? slab_candidate(P.half_z - z, dz, s_lim) : clamp0((P.half_z - z) / dz);
+  else if (dz < 0.0) s_z = filter ? slab_candidate(-P.half_z - z, dz, s_lim) : clamp0((-P.half_z - z) / dz);
   if (s_in <= s_out && s_in <= s_z) { which = HIT_INNER; return s_in; }
   if (s_out <= s_z) { which = HIT_OUTER; return s_out; }
   which = HIT_Z; return s_z;
