@@ -394,7 +394,8 @@ extern "C" int cel_create(const cel_geometry* g, const cel_material* mats, int n
   if (cudaEventCreate(&c->ev_start) != cudaSuccess || cudaEventCreate(&c->ev_stop) != cudaSuccess) return fail(CEL_ERR_CUDA);
   for (int i = 0; i < kStatusSlots; ++i)
     if (cudaEventCreateWithFlags(&c->ev_batch[i], cudaEventDisableTiming) != cudaSuccess) return fail(CEL_ERR_CUDA);
-  if (cudaMallocHost((void**)&c->h_status, kStatusSlots * sizeof(Control)) != cudaSuccess) return fail(CEL_ERR_OOM);
+  if (cudaHostAlloc((void**)&c->h_status, kStatusSlots * sizeof(Control), cudaHostAllocMapped) != cudaSuccess) return fail(CEL_ERR_OOM);
+  { void* dp = nullptr; if (cudaHostGetDevicePointer(&dp, c->h_status, 0) != cudaSuccess) return fail(CEL_ERR_CUDA); D.status_host = (Control*)dp; }
   *out = c;
   return CEL_OK;
 }
@@ -797,6 +798,7 @@ int prepare_run(cel_ctx* c, uint32_t n_events, bool debug) {
     CEL_CUDA(c, cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal));
     for (int b = 0; b < c->batch; ++b) c->kernels_per_iteration = enqueue_iteration(c);
     if (c->hits_mode) k_hits_batch_end<<<1, 1, 0, s>>>(c->D);
+    k_status<<<1, 64, 0, s>>>(c->D);
     CEL_CUDA(c, cudaStreamEndCapture(s, &c->graph));
     CEL_CUDA(c, cudaGraphInstantiate(&c->graph_exec, c->graph, 0));
     std::memcpy(&c->graph_D, &D, sizeof(DeviceState));
@@ -873,7 +875,7 @@ int run_loop(cel_ctx* c) {
     if (in_tail) {
       CEL_RANGE_PUSH("cel:tail_batch"); launch_tail(c); CEL_RANGE_POP();
       enqueued += c->tail_iters;
-      CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
+      k_status<<<1, 64, 0, s>>>(c->D); c->launches += 1;
       CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
       const int prev = slot ^ 1;
       CEL_CUDA(c, cudaEventSynchronize(c->ev_batch[prev]));
@@ -889,13 +891,14 @@ int run_loop(cel_ctx* c) {
     if (c->hits_mode == 1) consumer_wait_idle(c);
     if (c->graph_exec && c->use_graph && !c->profile && c->hits_mode != 2) {
       CEL_CUDA(c, cudaGraphLaunch(c->graph_exec, s));
-      c->launches += (uint64_t)c->kernels_per_iteration * c->batch + (c->hits_mode ? 1 : 0);
+      c->launches += (uint64_t)c->kernels_per_iteration * c->batch + (c->hits_mode ? 1 : 0) + 1;   // (+ k_status)
     } else {
       for (int b = 0; b < c->batch; ++b) {
         c->prof_b = b;
         per_iter = enqueue_iteration(c); c->launches += per_iter;
       }
       if (c->hits_mode) { k_hits_batch_end<<<1, 1, 0, s>>>(c->D); c->launches += 1; }
+      if (c->hits_mode != 2) { k_status<<<1, 64, 0, s>>>(c->D); c->launches += 1; }
     }
     c->prof_b = 0;
     enqueued += c->batch;
@@ -916,8 +919,7 @@ int run_loop(cel_ctx* c) {
       if (enqueued >= c->max_iterations) { rc = CEL_ERR_MAX_ITER; break; }
       continue;
     }
-    CEL_CUDA(c, cudaMemcpyAsync(&c->h_status[slot], c->D.ctl, sizeof(Control), cudaMemcpyDeviceToHost, s));
-    CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));
+    CEL_CUDA(c, cudaEventRecord(c->ev_batch[slot], s));   // (behind k_status, which has written h_status[slot])
     if (have_prev) {
       const int prev = slot ^ 1;
       CEL_CUDA(c, cudaEventSynchronize(c->ev_batch[prev]));

@@ -129,6 +129,7 @@ struct Control {
   unsigned long long hits_in_batch; // set by k_hits_batch_end: records of the batch that just ended ...
   uint32_t hits_buf;                // ... and the host ring buffer (0/1) they were streamed into
   uint32_t hits_cur;                // the host ring buffer the running batch streams into
+  uint32_t status_seq;              // batches whose status k_status has published to the host (its slot = status_seq & 1)
 };
 
 // one hit = one quantised deposit of one track in one iteration (S10): what the paper's application copies to the host
@@ -174,6 +175,7 @@ struct DeviceState {
   // (device-mapped) k_hits_flush streams it into; nullptr = off
   HitRec* hits; unsigned long long hit_capacity;
   HitRec* host_hits[2];
+  Control* status_host;   // [2] pinned, device-mapped: where k_status publishes the control block at the end of a batch of iterations
   // device-side timeline (option "trace", fig. 2): [trace_iters][K_COUNT][2] globaltimer ns, first block
   // in / last warp out of every kernel of every iteration; nullptr = off
   unsigned long long* trace;

@@ -849,6 +849,20 @@ __global__ void k_hits_batch_end(DeviceState D) {
   ctl->n_hits = 0; ctl->hits_mark[0] = 0; ctl->hits_mark[1] = 0;
 }
 
+// end of a batch of iterations: the control block straight into pinned host memory (the host loop never
+// blocks the device). An in-stream cudaMemcpyAsync of these 300 bytes cost ~10 us of copy-engine latency between two batches;
+// a one-warp kernel writing mapped memory costs ~2. Slots alternate with the batch count, as the host's own counter does.
+__global__ void k_status(DeviceState D) {
+  Control* ctl = D.ctl;
+  const uint32_t seq = ctl->status_seq;
+  uint32_t* dst = reinterpret_cast<uint32_t*>(D.status_host + (seq & 1u));
+  const uint32_t* src = reinterpret_cast<const uint32_t*>(ctl);
+  for (uint32_t i = threadIdx.x; i < sizeof(Control) / 4; i += blockDim.x) dst[i] = src[i];
+  __syncthreads();
+  if (threadIdx.x == 0) ctl->status_seq = seq + 1u;
+  __threadfence_system();
+}
+
 // ================================================================ loading, reset, debug helpers
 struct PrimaryRec { uint32_t event; int32_t ptype; double energy; double pos[3]; double dir[3]; };  // = cel_primary, 64 B
 struct TrackRec { double pos[3]; double dir[3]; double energy; uint32_t event, nsteps; int32_t vol, surf, ptype, action; };  // = cel_track
