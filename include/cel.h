@@ -115,7 +115,8 @@ int cel_set_workspace(cel_ctx*, void* dptr, uint64_t bytes);
 
 /* Transport: resets slots, tallies (sized n_events x (n_bins+1)) and counters, writes primary i to init[i]
  * (S9; primaries is a HOST array, validated, copied), then enqueues step iterations in batches on the stream
- * and returns when a lagged, asynchronously copied status word shows that no track and no initializer is left.
+ * and returns when a lagged copy of the control block (written into pinned host memory by a one-warp kernel at the end of every
+ * batch of iterations) shows that no track and no initializer is left.
  * The host never issues a synchronous copy or a device-wide synchronisation. */
 int cel_transport(cel_ctx*, const cel_primary* primaries, uint64_t n_primaries, uint32_t n_events);
 
